@@ -1,0 +1,261 @@
+"""Pins for the CPU oracle: the oracle is checked against closed forms,
+invariants, textbook special cases and an independent dense-array implementation -- never
+against itself and never against the CUDA path."""
+import itertools
+import math
+
+import numpy as np
+import pytest
+
+from oracle import dense_ctu
+from oracle.binding import Oracle
+
+S0 = 250813986
+
+
+def box(lo, hi):
+    """All integer coordinates c with lo <= c < hi (lexicographic)."""
+    return np.array(list(itertools.product(*[range(a, b) for a, b in zip(lo, hi)])), dtype=np.int32)
+
+
+def raw(n, h, dyn, params, keys, p, origin=None, cfl=0.9, hi_res=1, limiter=0, grow=False):
+    o = Oracle(n, h, 1e-300, dyn, params, cfl=cfl, hi_res=hi_res, limiter=limiter)
+    o.set_flags(grow=grow, normalise=False)
+    o.import_state(np.zeros(n) if origin is None else origin, keys, p)
+    return o
+
+
+def as_dict(keys, p):
+    return {tuple(k): v for k, v in zip(keys.tolist(), p.tolist())}
+
+
+# ---- P1 telescoping / conservation -------------------------------------------------------------
+@pytest.mark.parametrize("n,dyn,params", [(3, 0, [10, 8 / 3, 28]), (4, 2, [4.0]), (6, 2, [4.0])])
+def test_P1_conservation_when_support_is_two_cells_inside(n, dyn, params):
+    rng = np.random.default_rng(S0 + 101 + n)
+    side = {3: 9, 4: 7, 6: 5}[n]
+    keys = box([0] * n, [side] * n)
+    inner = np.all((keys >= 2) & (keys < side - 2), axis=1)
+    p = np.where(inner, rng.random(len(keys)), 0.0)
+    # ragged: drop a random 30% of the zero cells that are not within 2 cells of the support
+    o = raw(n, [0.5] * n, dyn, params, keys, p, origin=[1.0] * n)
+    o.step()
+    _, p1 = o.export()
+    assert abs(p1.sum() - p.sum()) <= len(keys) * 2.0 ** -52 * p.sum()
+    assert abs(o.last_mass() - p.sum()) <= len(keys) * 2.0 ** -52 * p.sum()
+
+
+def test_P1_mass_is_lost_only_through_boundary_faces():
+    # 1-D, u>0 everywhere, all cells carry mass: the only loss is the outflow of the last cell.
+    n, h, v = 1, [0.5], [1.0]
+    keys = box([0], [8])
+    p = np.arange(1, 9, dtype=np.float64)
+    o = raw(n, h, 4, v, keys, p, hi_res=0, cfl=0.5)
+    dt = o.step()
+    assert dt == 0.5 / (1.0 / 0.5)
+    _, p1 = o.export()
+    assert p1.sum() == pytest.approx(p.sum() - dt / 0.5 * 1.0 * p[-1], rel=1e-15)
+
+
+# ---- P2 Courant-1 shift, bit exact ----------------------------------------------------------------
+@pytest.mark.parametrize("n,axis,sign", [(1, 0, 1), (1, 0, -1), (3, 1, 1), (3, 2, -1), (6, 4, 1), (6, 0, -1)])
+def test_P2_courant_one_shift_is_bit_exact(n, axis, sign):
+    rng = np.random.default_rng(S0 + 102)
+    v = np.zeros(n)
+    v[axis] = 2.0 * sign
+    lo, hi = [0] * n, [3] * n
+    hi[axis] = 12
+    keys = box(lo, hi)
+    p = rng.integers(0, 64, len(keys)).astype(np.float64) * 2.0 ** -9
+    edge = (keys[:, axis] < 2) | (keys[:, axis] >= 10)
+    p[edge] = 0.0
+    for hi_res, limiter in [(0, 0), (1, 0), (1, 1)]:
+        o = raw(n, [0.5] * n, 4, v, keys, p, cfl=1.0, hi_res=hi_res, limiter=limiter)
+        dt = o.step()
+        assert dt == 0.25
+        k1, p1 = o.export()
+        d0, d1 = as_dict(keys, p), as_dict(k1, p1)
+        for k, val in d1.items():
+            src = list(k)
+            src[axis] -= sign
+            assert val == d0.get(tuple(src), 0.0)  # bit exact
+
+
+# ---- P3 n-D constant-velocity closed form, all 2^n sign patterns ---------------------------------
+def closed_form_ctu(P, nu, sgn):
+    """P' = P - sum_j nu_j D_j P + sum_{j<l} nu_j nu_l D_j D_l P, D_j = upwind difference."""
+    n = P.ndim
+
+    def D(A, j):
+        return A - np.roll(A, sgn[j], axis=j)
+
+    out = P.copy()
+    for j in range(n):
+        out = out - nu[j] * D(P, j)
+    for j in range(n):
+        for l in range(j + 1, n):
+            out = out + nu[j] * nu[l] * D(D(P, j), l)
+    return out
+
+
+@pytest.mark.parametrize("n,side", [(2, 9), (3, 7), (6, 5)])
+def test_P3_constant_velocity_closed_form_all_sign_patterns(n, side):
+    rng = np.random.default_rng(S0 + 103 + n)
+    h = np.array([0.5, 0.25, 1.0, 0.5, 2.0, 0.75][:n])
+    keys = box([0] * n, [side] * n)
+    Pd = np.zeros([side] * n)
+    inner = tuple([slice(2, side - 2)] * n)
+    Pd[inner] = rng.random(Pd[inner].shape)
+    p = Pd[tuple(keys.T)]
+    for sgn in itertools.product([1, -1], repeat=n):
+        speed = rng.uniform(0.3, 1.5, n)
+        v = speed * np.array(sgn)
+        o = raw(n, h, 4, v, keys, p, cfl=0.9, hi_res=0)
+        dt = o.step()
+        nu = speed * dt / h
+        assert nu.sum() == pytest.approx(0.9, rel=1e-14)
+        k1, p1 = o.export()
+        got = np.zeros_like(Pd)
+        got[tuple(k1.T)] = p1
+        want = closed_form_ctu(Pd, nu, sgn)
+        sl = tuple([slice(1, side - 1)] * n)
+        assert np.max(np.abs(got[sl] - want[sl])) <= 1e-14 * np.max(np.abs(want))
+
+
+# ---- P4 1-D DCU binomial smear ------------------------------------------------------------------------
+def test_P4_dcu_binomial_smear():
+    N, k, nu = 64, 10, 0.4
+    keys = box([0], [N])
+    p = np.where((keys[:, 0] >= 10) & (keys[:, 0] < 20), 1.0, 0.0)
+    o = raw(1, [0.5], 4, [1.0], keys, p, hi_res=0, cfl=1.0)
+    for _ in range(k):
+        assert o.step(nu * 0.5) == nu * 0.5
+    _, p1 = o.export()
+    want = np.zeros(N)
+    for m in range(k + 1):
+        w = math.comb(k, m) * nu ** m * (1 - nu) ** (k - m)
+        want[m:] += w * p[: N - m]
+    assert np.max(np.abs(p1 - want)) < 1e-13
+
+
+# ---- P5 Lax-Wendroff with phi == 1 ---------------------------------------------------------------------
+@pytest.mark.parametrize("sign", [1, -1])
+def test_P5_unlimited_hires_is_lax_wendroff(sign):
+    rng = np.random.default_rng(S0 + 105)
+    N, nu = 40, 0.37
+    keys = box([0], [N])
+    p = np.zeros(N)
+    p[5:35] = rng.random(30)
+    o = raw(1, [0.25], 4, [2.0 * sign], keys, p, hi_res=1, limiter=1, cfl=1.0)
+    dt = nu * 0.25 / 2.0
+    assert o.step(dt) == dt
+    _, p1 = o.export()
+    c = nu * sign
+    want = p - c / 2 * (np.roll(p, -1) - np.roll(p, 1)) + c * c / 2 * (np.roll(p, -1) - 2 * p + np.roll(p, 1))
+    assert np.max(np.abs(p1[2:-2] - want[2:-2])) < 1e-14
+
+
+# ---- P6 MC limiter: TVD and order of accuracy --------------------------------------------------------
+def test_P6_mc_limiter_is_tvd_on_step_data():
+    N = 80
+    keys = box([0], [N])
+    p = np.where((keys[:, 0] >= 10) & (keys[:, 0] < 30), 1.0, 0.0)
+    o = raw(1, [0.5], 4, [1.0], keys, p, hi_res=1, limiter=0, cfl=0.8)
+    tv = np.abs(np.diff(p)).sum()
+    for _ in range(40):
+        o.step()
+        _, p1 = o.export()
+        tv1 = np.abs(np.diff(p1)).sum()
+        assert tv1 <= tv * (1 + 1e-14)
+        tv = tv1
+        assert p1.min() >= -1e-15 and p1.max() <= 1 + 1e-14
+
+
+def _advect_gaussian_error(N, hi_res):
+    h, v, nu, L = 1.0 / N, 1.0, 0.8, 1.0
+    keys = box([-2 * N], [4 * N])
+    x = keys[:, 0] * h
+    f = lambda y: np.exp(-0.5 * ((y - 0.5) / 0.08) ** 2)
+    o = raw(1, [h], 4, [v], keys, f(x), hi_res=hi_res, cfl=1.0)
+    steps = int(round(L / (nu * h)))
+    for _ in range(steps):
+        o.step(nu * h / v)
+    _, p1 = o.export()
+    return h * np.abs(p1 - f(x - v * o.time())).sum()
+
+
+def test_P6_second_order_with_hires_first_order_without():
+    e1, e2 = _advect_gaussian_error(100, 1), _advect_gaussian_error(200, 1)
+    assert 1.7 <= math.log2(e1 / e2) <= 2.3
+    f1, f2 = _advect_gaussian_error(100, 0), _advect_gaussian_error(200, 0)
+    assert 0.6 <= math.log2(f1 / f2) <= 1.2
+    assert e2 < f2 / 10
+
+
+# ---- P7 brute force: dense gather form vs sparse scatter form ---------------------------------------
+CASES_P7 = [
+    (3, 6, 0, [10, 8 / 3, 28], [-11.5, -10, 9.5]),
+    (3, 6, 1, [4.0, 1.0, 48.0], [-11.5, -10, 9.5]),
+    (4, 4, 2, [4.0], [4.01, 4, 4, 4]),
+    (6, 3, 2, [4.0], [4.01, 4, 4, 4, 4, 4]),
+    (6, 3, 3, None, [0.3, -0.2, 0.1, 0.5, -0.4, 0.2]),
+]
+
+
+@pytest.mark.parametrize("n,side,dyn,params,origin", CASES_P7)
+@pytest.mark.parametrize("ragged", [False, True])
+def test_P7_dense_gather_form_equals_sparse_scatter_form(n, side, dyn, params, origin, ragged):
+    rng = np.random.default_rng(S0 + 107 + 10 * n + dyn + ragged)
+    if params is None:
+        params = rng.normal(0, 0.3, (n, n)).ravel()
+    h = rng.uniform(0.3, 0.6, n)
+    keys = box([-(side // 2)] * n, [side - side // 2] * n)
+    if ragged:
+        keys = keys[rng.random(len(keys)) < 0.6]
+    p = rng.random(len(keys)) - 0.1  # a few negatives: no clipping anywhere (A5)
+    order = np.lexsort(keys.T[::-1])
+    keys, p = keys[order], p[order]
+    for hi_res, limiter in [(0, 0), (1, 0), (1, 1)]:
+        o = raw(n, h, dyn, params, keys, p, origin=origin, hi_res=hi_res, limiter=limiter)
+        dt = o.step()
+        k1, p1 = o.export()
+        assert np.array_equal(k1, keys)
+        want = dense_ctu.dense_step_sparse(keys, p, dyn, params, origin, h, dt, bool(hi_res), limiter)
+        assert np.max(np.abs(p1 - want)) <= 1e-13 * np.max(np.abs(want))
+
+
+# ---- P8 dt closed forms (Eq. 8) --------------------------------------------------------------------------
+def test_P8_dt_constant_velocity_exact():
+    v, h = [1.5, -0.25, 3.0], [0.5, 0.125, 2.0]
+    o = raw(3, h, 4, v, box([0] * 3, [3] * 3), np.ones(27), cfl=0.9)
+    assert o.step() == 0.9 / (1.5 / 0.5 + 0.25 / 0.125 + 3.0 / 2.0)
+    assert o.step(1e-3) == 1e-3  # caller's cap binds
+    assert o.step(float("inf")) == 0.9 / 6.5 and o.step(-1.0) == 0.9 / 6.5
+
+
+def test_P8_dt_linear_dynamics_brute_force():
+    rng = np.random.default_rng(S0 + 108)
+    n, A = 3, rng.normal(0, 0.3, (3, 3))
+    h, origin = np.array([0.5, 0.4, 0.3]), np.array([0.2, -0.1, 0.3])
+    keys = box([-4, -3, -5], [5, 4, 3])
+    o = raw(n, h, 3, A.ravel(), keys, np.ones(len(keys)), origin=origin, cfl=0.9)
+    s = np.zeros(len(keys))
+    for j in range(n):
+        xf = origin + keys * h
+        xf[:, j] -= 0.5 * h[j]
+        s += np.abs(xf @ A[j]) / h[j]
+    assert o.step() == pytest.approx(0.9 / s.max(), rel=1e-15)
+
+
+def test_A12_face_velocity_matches_independent_numpy():
+    rng = np.random.default_rng(S0 + 112)
+    for n, dyn, params in [(3, 0, [10, 8 / 3, 28]), (3, 1, [4, 1, 48]), (6, 2, [4.0]), (4, 2, [8.0]),
+                           (5, 3, rng.normal(0, 0.3, 25))]:
+        h, origin = rng.uniform(0.2, 0.6, n), rng.normal(0, 3, n)
+        o = raw(n, h, dyn, params, np.zeros((1, n), dtype=np.int32), [1.0], origin=origin)
+        for _ in range(20):
+            c = rng.integers(-30, 30, n).astype(np.int32)
+            for j in range(n):
+                x = [np.float64(origin[m] + (c[m] - (0.5 if m == j else 0.0)) * h[m]) for m in range(n)]
+                want = float(dense_ctu.dynamics(dyn, params, x, j))
+                assert o.face_velocity(c, j) == pytest.approx(want, rel=1e-13, abs=1e-13)
