@@ -259,3 +259,160 @@ def test_A12_face_velocity_matches_independent_numpy():
                 x = [np.float64(origin[m] + (c[m] - (0.5 if m == j else 0.0)) * h[m]) for m in range(n)]
                 want = float(dense_ctu.dynamics(dyn, params, x, j))
                 assert o.face_velocity(c, j) == pytest.approx(want, rel=1e-13, abs=1e-13)
+
+
+# ---- P9 linear dynamics: grid moments follow N(e^{At} mu, e^{At} Sigma e^{A^T t}) ---------------------
+def _moments(keys, p, origin, h):
+    x = origin + keys * h
+    m = (p[:, None] * x).sum(0)
+    d = x - m
+    return m, (p[:, None, None] * d[:, :, None] * d[:, None, :]).sum(0)
+
+
+def _expm(A, t):
+    w, V = np.linalg.eig(A)
+    return (V @ np.diag(np.exp(w * t)) @ np.linalg.inv(V)).real
+
+
+def test_P9_linear_dynamics_moments_full_pipeline():
+    A = np.array([[-0.1, 1.0], [-1.0, -0.2]])
+    mu0, cov0, T = np.array([2.0, 0.5]), np.array([[0.09, 0.02], [0.02, 0.05]]), 0.8
+    errs = []
+    for dx in (0.06, 0.03):
+        o = Oracle(2, [dx, dx], 1e-9, 3, A.ravel(), cfl=0.9)
+        o.init_gaussian(mu0, cov0)
+        k = 0
+        while o.time() < T:
+            o.step(T - o.time())
+            k += 1
+            if k % 3 == 0:
+                o.prune()
+        keys, p = o.export()
+        assert p.sum() == pytest.approx(1.0, abs=1e-12)
+        m, S = _moments(keys, p, mu0, np.array([dx, dx]))
+        E = _expm(A, T)
+        errs.append((np.abs(m - E @ mu0).max(), np.abs(S - E @ cov0 @ E.T).max() / np.abs(cov0).max()))
+    assert errs[1][0] < 2e-3 and errs[1][1] < 0.02      # discretisation-limited
+    assert errs[1][1] < errs[0][1] / 2.5                # improves ~4x per halving (2nd order)
+
+
+# ---- P10 correction: direct Bayes product and Kalman moments -----------------------------------------------
+def test_P10_correction_direct_and_kalman():
+    n, dx = 3, 0.2
+    mu0, cov0 = np.array([-11.5, -10, 9.5]), np.diag([1.0, 0.5, 0.8])
+    z, R = np.array([-11.0, -10.4, 9.9]), np.array([[1.0, 0.2, 0], [0.2, 0.7, 0.1], [0, 0.1, 1.2]])
+    o = Oracle(n, [dx] * n, 1e-9, 0, [10, 8 / 3, 28])
+    o.init_gaussian(mu0, cov0)
+    keys, p0 = o.export()
+    o.correct(z, R)
+    k1, p1 = o.export()
+    assert np.array_equal(keys, k1)
+    d = z - (mu0 + keys * dx)
+    L = np.exp(-0.5 * np.einsum("ij,jk,ik->i", d, np.linalg.inv(R), d))
+    want = p0 * L / (p0 * L).sum()
+    assert np.max(np.abs(p1 - want)) <= 1e-13 * want.max()  # summation order over 47k cells
+    K = cov0 @ np.linalg.inv(cov0 + R)
+    m, S = _moments(keys, p1, mu0, np.array([dx] * n))
+    assert np.abs(m - (mu0 + K @ (z - mu0))).max() < 2e-3
+    assert np.abs(S - (np.eye(n) - K) @ cov0).max() < 5e-3
+
+
+def test_A8_init_gaussian_set_and_values():
+    n, dx, thr = 3, 0.5, 2e-5
+    cov = np.array([[1.0, 0.3, 0.0], [0.3, 0.8, -0.2], [0.0, -0.2, 1.1]])
+    o = Oracle(n, [dx] * n, thr, 0, [10, 8 / 3, 28])
+    o.init_gaussian([-11.5, -10, 9.5], cov)
+    keys, p = o.export()
+    cand = box([-14] * 3, [15] * 3)
+    d = cand * dx
+    g = np.exp(-0.5 * np.einsum("ij,jk,ik->i", d, np.linalg.inv(cov), d)) * dx ** 3 / np.sqrt(
+        (2 * np.pi) ** 3 * np.linalg.det(cov))
+    sel = g >= thr
+    assert np.array_equal(keys, cand[sel])
+    assert np.max(np.abs(p - g[sel] / g[sel].sum())) < 1e-15
+    # BASELINE config 0 / config 2 initial sets (sizes quoted in SURVEY.md 8(a))
+    o.init_gaussian([-11.5, -10, 9.5], np.eye(3))
+    assert o.count() == 1357
+
+
+# ---- P12 grow / prune duality (independent python statement of Targets, D1.1 / D3) ------------------------
+def py_targets(c, dyn, params, origin, h):
+    n = len(c)
+
+    def u(cell, j):
+        x = [np.float64(origin[m] + (cell[m] - (0.5 if m == j else 0.0)) * h[m]) for m in range(n)]
+        return float(dense_ctu.dynamics(dyn, params, x, j))
+
+    out = {}
+    for j in range(n):
+        up = list(c)
+        up[j] += 1
+        if u(up, j) > 0:
+            out[j] = out.get(j, []) + [+1]
+        if u(c, j) < 0:
+            out[j] = out.get(j, []) + [-1]
+    tg = set()
+    for j, ss in out.items():
+        for s in ss:
+            t = list(c); t[j] += s; tg.add(tuple(t))
+            for l, sl in out.items():
+                if l > j:
+                    for s2 in sl:
+                        t2 = list(t); t2[l] += s2; tg.add(tuple(t2))
+    return tg
+
+
+@pytest.mark.parametrize("n,dyn,params,mean,cov,dx,thr", [
+    (3, 0, [10, 8 / 3, 28], [-11.5, -10, 9.5], 1.0, 0.5, 2e-5),
+    (4, 2, [4.0], [4.01, 4, 4, 4], 0.25, 0.5, 1e-5),
+])
+def test_P12_grow_prune_duality(n, dyn, params, mean, cov, dx, thr):
+    h = [dx] * n
+    o = Oracle(n, h, thr, dyn, params)
+    o.init_gaussian(mean, cov * np.eye(n))
+    for it in range(3):
+        k0, p0 = o.export()
+        o.step()
+        k1, p1 = o.export()
+        set1 = set(map(tuple, k1.tolist()))
+        assert len(set1) == len(k1)                      # no key twice
+        want = set(map(tuple, k0.tolist()))
+        for c in k0[p0 >= thr].tolist():
+            tg = py_targets(c, dyn, params, mean, h)
+            assert tg == set(map(tuple, o.targets(c).tolist()))
+            want |= tg
+        assert set1 == want                              # grow = exactly I u Targets(S)
+        o.prune()
+        k2, p2 = o.export()
+        keep = set()
+        for c in k1[p1 >= thr].tolist():
+            keep.add(tuple(c))
+            keep |= py_targets(c, dyn, params, mean, h) & set1
+        assert set(map(tuple, k2.tolist())) == keep      # D3
+        assert p2.sum() == pytest.approx(1.0, abs=1e-13)
+        o.prune()
+        k3, _ = o.export()
+        assert np.array_equal(k2, k3)                    # prune is idempotent
+
+
+# ---- P13 reflection symmetry -------------------------------------------------------------------------------
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_P13_reflection(axis):
+    rng = np.random.default_rng(S0 + 113)
+    n, A = 3, rng.normal(0, 0.5, (3, 3))
+    h, origin = np.array([0.5, 0.4, 0.3]), np.array([0.2, -0.1, 0.3])
+    keys = box([-3] * 3, [4] * 3)
+    keys = keys[rng.random(len(keys)) < 0.7]
+    p = rng.random(len(keys))
+    M = np.eye(3); M[axis, axis] = -1
+    o1 = raw(n, h, 3, A.ravel(), keys, p, origin=origin)
+    o2 = raw(n, h, 3, (M @ A @ M).ravel(), keys * M.diagonal().astype(np.int32), p, origin=M @ origin)
+    # Eq. (8) as printed uses the LOWER faces only (reading A4), which a reflection maps to upper
+    # faces: dt itself is not mirror-symmetric, so both runs take the same capped step.
+    for _ in range(2):
+        assert o1.step(0.05) == 0.05 and o2.step(0.05) == 0.05
+    k1, p1 = o1.export(); k2, p2 = o2.export()
+    d1 = as_dict(k1, p1)
+    d2 = as_dict(k2 * M.diagonal().astype(np.int32), p2)
+    assert d1.keys() == d2.keys()
+    assert max(abs(d1[k] - d2[k]) for k in d1) <= 1e-14 * p1.max()
