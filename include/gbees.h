@@ -1,0 +1,134 @@
+/* gbees.h -- C ABI of the B200-native GBEES prediction step (arXiv 2508.13986, "GBEES-GPU").
+ *
+ * The library advances a probability density on a sparse, dynamically allocated n-D grid under
+ * dp/dt + div(f p) = 0 (Eq. 3) with the Corner Transport Upwind finite-volume scheme
+ * (Eq. 7, Alg. 1, PAPER.md:112 high-resolution terms), growing the
+ * grid downwind of above-threshold cells and pruning cells below threshold,
+ * with the Bayes correction of PAPER.md:59 (Eq. 4). Exact semantics: DESIGN.md "Definitions D1-D5".
+ *
+ * Conventions
+ *  - Every call returns 0 (GBEES_OK) or a negative GBEES_ERR_*; nothing throws or aborts across
+ *    the ABI. Device-side faults (pool overflow, key range) are recorded in a device flag and
+ *    surfaced by the call that detected them; gbees_last_error() gives a message.
+ *  - All computation happens in CUDA kernels on one GPU (sm_100a). There is no CPU fallback.
+ *  - "host" / "device" below says where a pointer must live. Arrays passed in are copied; the
+ *    caller keeps ownership of everything it passes. One context = one stream; calls on one
+ *    context are not re-entrant.
+ *  - Cell c in Z^n has centre x_c = origin + c o dx; origin = the mean given to init_gaussian.
+ *    P_c is the probability MASS of cell c; sum over active cells = 1 after every normalisation.
+ */
+#ifndef GBEES_H
+#define GBEES_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GBEES_OK 0
+#define GBEES_ERR_ARG (-1)        /* bad argument (n out of [1,6], dx <= 0, wrong n_params, NULL) */
+#define GBEES_ERR_CUDA (-2)       /* a CUDA runtime call failed (message in gbees_last_error) */
+#define GBEES_ERR_NOT_SPD (-3)    /* cov / R is not symmetric positive definite */
+#define GBEES_ERR_CAPACITY (-4)   /* more cells than opts.max_cells (fixed capacity) */
+#define GBEES_ERR_BUFFER (-5)     /* export buffer too small; *count holds the needed size */
+#define GBEES_ERR_DEGENERATE (-6) /* mass <= 0 or non-finite, empty grid, or no CFL bound and no cap */
+#define GBEES_ERR_KEY_RANGE (-7)  /* a coordinate left the packable range (floor(63/n) bits, biased) */
+
+/* dynamics ids: f(x) in dx/dt = f(x). Operation order is fixed (A12). */
+#define GBEES_DYN_LORENZ63 0        /* params (sigma, beta, rho); n = 3 (BASELINE configs 0-1) */
+#define GBEES_DYN_LORENZ63_PAPER 1  /* params (sigma, b, r), PAPER.md:303 z-shifted form; n = 3 */
+#define GBEES_DYN_LORENZ96 2        /* params (F); n >= 4, cyclic */
+#define GBEES_DYN_LINEAR 3          /* params A row-major n*n: f = A x (BASELINE config 3) */
+#define GBEES_DYN_CONSTANT 4        /* params v[n]: f = v (tests) */
+
+typedef struct gbees_ctx gbees_ctx;
+
+typedef struct gbees_opts {
+    int64_t max_cells;   /* pool capacity; hashtable has ceil(max_cells / load_factor) slots */
+    double load_factor;  /* default 0.5 */
+    double cfl;          /* C in dt = C * min_c (sum_j |u_cj| / h_j)^-1, Eq. (8); default 0.9 */
+    int hi_res;          /* 1 = add the high-resolution (limited Lax-Wendroff) term; default 1 */
+    int limiter;         /* 0 = monotonised central, 1 = none (phi == 1, test mode) */
+    int no_grow;         /* test mode: gbees_step does not grow the grid */
+    int no_normalise;    /* test mode: keep raw (un-normalised) masses after step / prune */
+    int device;          /* CUDA device ordinal */
+    void* stream;        /* cudaStream_t to run on (e.g. torch's current stream); NULL = default */
+} gbees_opts;
+
+typedef struct gbees_stats_t {
+    int64_t n_cells;        /* active cells now */
+    int64_t n_inserted;     /* cells created by the last step's grow */
+    int64_t n_pruned;       /* cells removed by the last prune */
+    int64_t steps;          /* steps taken since init */
+    double t;               /* simulated time */
+    double dt;              /* last step size */
+    double mass;            /* mass before the last normalisation (1 - mass left the grid) */
+    int64_t cell_updates;   /* sum over steps of the active-cell count after grow */
+    int64_t table_slots;    /* hashtable capacity in slots */
+} gbees_stats_t;
+
+/* Fill *opts with the defaults (max_cells = 1<<20, load_factor 0.5, cfl 0.9, hi_res 1, MC). */
+int gbees_default_opts(gbees_opts* opts /*host*/);
+
+/* Allocate all fixed-capacity device structures. dx, params: host, copied.
+ * n in [1,6]; n_params must match dynamics_id. opts may be NULL (defaults). */
+int gbees_create(gbees_ctx** out, int n, const double* dx /*host [n]*/, double threshold,
+                 int dynamics_id, const double* params /*host*/, int n_params,
+                 const gbees_opts* opts /*host, nullable*/);
+int gbees_destroy(gbees_ctx* ctx);
+
+/* DESIGN.md D5/A8: origin <- mean, grid <- {c : g_c * prod(dx) / sqrt((2 pi)^n det cov) >= threshold},
+ * P <- normalised, t <- 0. mean [n], cov [n*n row-major, SPD]: host. */
+int gbees_init_gaussian(gbees_ctx* ctx, const double* mean, const double* cov);
+
+/* Raw state import (tests / restart): origin [n] host; keys [count*n] int32 row-major and p [count]
+ * on host or device. Keys must be distinct. P is taken as given (no normalisation), t <- 0. */
+int gbees_import(gbees_ctx* ctx, const double* origin, const int32_t* keys, const double* p, int64_t count);
+
+/* One prediction step, D1: grow -> dt (Eq. 8) -> CTU flux -> update -> normalise.
+ * in: *dt = largest step allowed (<= 0, NaN or inf = unconstrained); out: *dt = step taken.
+ * dt: host pointer. Does not prune. */
+int gbees_step(gbees_ctx* ctx, double* dt);
+
+/* DESIGN.md D3 (Alg. 3): keep cells with P >= threshold and the grow-targets of such
+ * cells; stream-compact the pool, rebuild the hashtable, renormalise. */
+int gbees_prune(gbees_ctx* ctx);
+
+/* DESIGN.md D4, Eq. (4): P_c <- P_c * exp(-1/2 (z - x_c)^T R^-1 (z - x_c)), renormalise.
+ * z [n], R [n*n row-major SPD]: host. Does not prune. */
+int gbees_correct(gbees_ctx* ctx, const double* z, const double* R);
+
+/* Write the active cells in unspecified order: keys [cap*n] int32 row-major, p [cap] (normalised).
+ * Buffers: host or device (detected), caller-owned. keys == NULL and p == NULL: only *count.
+ * cap < count: nothing written, *count = needed, GBEES_ERR_BUFFER. count: host pointer. */
+int gbees_export(gbees_ctx* ctx, int32_t* keys, double* p, int64_t cap, int64_t* count);
+
+/* Persistent step loop: advance until t == t_target or max_steps steps, pruning
+ * after every prune_every-th step (0 = never). Observationally identical to the same sequence of
+ * gbees_step(&cap = t_target - t) / gbees_prune calls. steps_done: host, nullable. */
+int gbees_run(gbees_ctx* ctx, double t_target, int64_t max_steps, int prune_every, int64_t* steps_done);
+
+int gbees_count(gbees_ctx* ctx, int64_t* count /*host*/);
+int gbees_time(gbees_ctx* ctx, double* t /*host*/);
+int gbees_stats(gbees_ctx* ctx, gbees_stats_t* out /*host*/);
+const char* gbees_last_error(gbees_ctx* ctx);
+int gbees_clear_error(gbees_ctx* ctx);
+
+/* ---- BASELINE config 4: hashtable / compaction microbenchmark on the same device code ---------
+ * Keys are packed 64-bit values (never all-ones) in DEVICE memory. probes = slots inspected. */
+typedef struct gbees_ht gbees_ht;
+int gbees_ht_create(gbees_ht** out, int64_t slots, int device);
+int gbees_ht_destroy(gbees_ht* ht);
+/* insert-if-absent keys[0..k); idx_out[i] = pool index assigned (or existing); nullable */
+int gbees_ht_insert(gbees_ht* ht, const uint64_t* keys, int64_t k, uint32_t* idx_out, uint64_t* probes /*host*/);
+/* out[i] = pool index of query[i] or 0xFFFFFFFF */
+int gbees_ht_lookup(gbees_ht* ht, const uint64_t* query, int64_t k, uint32_t* out, uint64_t* probes /*host*/);
+/* delete keys[i] where del[i] != 0: decoupled-lookback scan + stable compaction of keys (in place)
+ * + table rebuild. *k_out = survivors. */
+int gbees_ht_compact(gbees_ht* ht, uint64_t* keys, const uint8_t* del, int64_t k, int64_t* k_out /*host*/);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GBEES_H */

@@ -1,0 +1,173 @@
+"""ctypes binding with the same names as include/gbees.h (argument marshalling only)."""
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(HERE, "libgbees.so")
+_lib = None
+
+ERRORS = {-1: "ARG", -2: "CUDA", -3: "NOT_SPD", -4: "CAPACITY", -5: "BUFFER", -6: "DEGENERATE", -7: "KEY_RANGE"}
+
+
+class GbeesError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"gbees error {code} ({ERRORS.get(code, '?')}): {msg}")
+        self.code = code
+
+
+class Opts(C.Structure):
+    _fields_ = [("max_cells", C.c_int64), ("load_factor", C.c_double), ("cfl", C.c_double),
+                ("hi_res", C.c_int), ("limiter", C.c_int), ("no_grow", C.c_int), ("no_normalise", C.c_int),
+                ("device", C.c_int), ("stream", C.c_void_p)]
+
+
+class Stats(C.Structure):
+    _fields_ = [("n_cells", C.c_int64), ("n_inserted", C.c_int64), ("n_pruned", C.c_int64), ("steps", C.c_int64),
+                ("t", C.c_double), ("dt", C.c_double), ("mass", C.c_double), ("cell_updates", C.c_int64),
+                ("table_slots", C.c_int64)]
+
+
+def lib_path():
+    return _LIB_PATH
+
+
+def lib():
+    """Load libgbees.so. Fails loudly when the CUDA extension has not been built."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise ImportError(f"{_LIB_PATH} is missing: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(_LIB_PATH)
+        vp, dp, ip = C.c_void_p, C.POINTER(C.c_double), C.c_void_p
+        L.gbees_default_opts.argtypes = [C.POINTER(Opts)]
+        L.gbees_create.argtypes = [C.POINTER(vp), C.c_int, dp, C.c_double, C.c_int, dp, C.c_int, C.POINTER(Opts)]
+        L.gbees_destroy.argtypes = [vp]
+        L.gbees_init_gaussian.argtypes = [vp, dp, dp]
+        L.gbees_import.argtypes = [vp, dp, ip, C.c_void_p, C.c_int64]
+        L.gbees_step.argtypes = [vp, dp]
+        L.gbees_prune.argtypes = [vp]
+        L.gbees_correct.argtypes = [vp, dp, dp]
+        L.gbees_export.argtypes = [vp, C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(C.c_int64)]
+        L.gbees_run.argtypes = [vp, C.c_double, C.c_int64, C.c_int, C.POINTER(C.c_int64)]
+        L.gbees_count.argtypes = [vp, C.POINTER(C.c_int64)]
+        L.gbees_time.argtypes = [vp, dp]
+        L.gbees_stats.argtypes = [vp, C.POINTER(Stats)]
+        L.gbees_last_error.argtypes = [vp]
+        L.gbees_last_error.restype = C.c_char_p
+        L.gbees_clear_error.argtypes = [vp]
+        _lib = L
+    return _lib
+
+
+def _d(a):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a, a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+class Gbees:
+    """One GBEES context on one GPU. Methods mirror the C ABI one to one."""
+
+    def __init__(self, n, dx, threshold, dynamics_id, params, max_cells=1 << 20, load_factor=0.5, cfl=0.9,
+                 hi_res=1, limiter=0, no_grow=False, no_normalise=False, device=0, stream=None):
+        L = lib()
+        self.n = int(n)
+        o = Opts()
+        L.gbees_default_opts(C.byref(o))
+        o.max_cells, o.load_factor, o.cfl = int(max_cells), float(load_factor), float(cfl)
+        o.hi_res, o.limiter, o.no_grow, o.no_normalise = int(hi_res), int(limiter), int(no_grow), int(no_normalise)
+        o.device = int(device)
+        o.stream = C.c_void_p(stream) if stream else None
+        self._h = C.c_void_p()
+        _, dxp = _d(dx)
+        par, pp = _d(params)
+        rc = L.gbees_create(C.byref(self._h), self.n, dxp, float(threshold), int(dynamics_id), pp, int(par.size),
+                            C.byref(o))
+        if rc:
+            self._h = None
+            raise GbeesError(rc, "gbees_create failed")
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().gbees_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def _chk(self, rc):
+        if rc:
+            raise GbeesError(rc, lib().gbees_last_error(self._h).decode())
+
+    def init_gaussian(self, mean, cov):
+        _, m = _d(mean)
+        _, c = _d(cov)
+        self._chk(lib().gbees_init_gaussian(self._h, m, c))
+
+    def import_state(self, origin, keys, p):
+        """keys/p: numpy arrays (host) or torch CUDA tensors (device pointers are passed through)."""
+        _, o = _d(origin)
+        if hasattr(keys, "data_ptr"):
+            kp, pp, cnt = keys.data_ptr(), p.data_ptr(), int(p.numel())
+            hold = (keys, p)
+        else:
+            ka = np.ascontiguousarray(keys, dtype=np.int32).reshape(-1, self.n)
+            pa = np.ascontiguousarray(p, dtype=np.float64)
+            kp, pp, cnt, hold = ka.ctypes.data, pa.ctypes.data, int(pa.size), (ka, pa)
+        self._chk(lib().gbees_import(self._h, o, kp, pp, cnt))
+        del hold
+
+    def step(self, dt_cap=0.0):
+        dt = C.c_double(float(dt_cap))
+        self._chk(lib().gbees_step(self._h, C.byref(dt)))
+        return dt.value
+
+    def prune(self):
+        self._chk(lib().gbees_prune(self._h))
+
+    def correct(self, z, R):
+        _, zp = _d(z)
+        _, rp = _d(R)
+        self._chk(lib().gbees_correct(self._h, zp, rp))
+
+    def run(self, t_target, max_steps=1 << 62, prune_every=0):
+        done = C.c_int64()
+        self._chk(lib().gbees_run(self._h, float(t_target), int(max_steps), int(prune_every), C.byref(done)))
+        return done.value
+
+    def count(self):
+        n = C.c_int64()
+        self._chk(lib().gbees_count(self._h, C.byref(n)))
+        return n.value
+
+    def time(self):
+        t = C.c_double()
+        self._chk(lib().gbees_time(self._h, C.byref(t)))
+        return t.value
+
+    def stats(self):
+        s = Stats()
+        self._chk(lib().gbees_stats(self._h, C.byref(s)))
+        return {k: getattr(s, k) for k, _ in Stats._fields_}
+
+    def last_mass(self):
+        return self.stats()["mass"]
+
+    def export(self, sort=True):
+        """Host export: (keys int32 [N,n], p float64 [N]); sorted lexicographically if sort."""
+        N = self.count()
+        keys = np.empty((N, self.n), dtype=np.int32)
+        p = np.empty(N, dtype=np.float64)
+        cnt = C.c_int64()
+        self._chk(lib().gbees_export(self._h, keys.ctypes.data, p.ctypes.data, N, C.byref(cnt)))
+        if sort and N:
+            order = np.lexsort(keys.T[::-1])
+            keys, p = keys[order], p[order]
+        return keys, p
+
+    def export_device(self, keys_t, p_t):
+        """Device export into caller-owned torch CUDA tensors (int32 [cap,n], float64 [cap])."""
+        cnt = C.c_int64()
+        self._chk(lib().gbees_export(self._h, keys_t.data_ptr(), p_t.data_ptr(), int(p_t.numel()), C.byref(cnt)))
+        return cnt.value

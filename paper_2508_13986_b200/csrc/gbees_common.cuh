@@ -1,0 +1,194 @@
+// Device-side building blocks of the GBEES prediction step (sm_100a): key packing, hashtable,
+// dynamics / face velocities. See DESIGN.md for layout and semantics; citations are PAPER.md lines.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace gbees {
+
+constexpr int MAXN = 6;
+constexpr uint64_t KEY_EMPTY = ~0ull;            // all-ones is never a packed key (A18)
+constexpr uint64_t KEY_GROWN = 1ull << 63;       // pool-only flag: Targets(c) already inserted
+constexpr uint32_t NBR_NONE = 0xFFFFFFFFu;       // no neighbour, direct or two-hop
+constexpr uint32_t NBR_TAG = 0x80000000u;        // direct neighbour missing; low bits = two-hop cell
+
+enum ErrBits : int { E_CAPACITY = 1, E_KEY_RANGE = 2, E_DEGENERATE = 4, E_TABLE_FULL = 8 };
+
+// Launch-invariant problem description, passed by value (__grid_constant__) to every kernel.
+struct Params {
+    int n;
+    int dyn;
+    int bits;            // bits per coordinate field = min(floor(63/n), 31)
+    int hi_res;
+    int limiter;
+    int normalise;
+    int64_t bias;        // 2^(bits-1)
+    double h[MAXN];
+    double mu[MAXN];     // grid origin
+    double par[MAXN * MAXN];
+    double thresh;
+    double cfl;
+    uint32_t cap;        // pool capacity (cells)
+    uint64_t slots;      // hashtable slots
+};
+
+// Mutable scalars living in device memory (one struct, read back after each API call).
+struct DevState {
+    uint32_t N;                 // active cells
+    uint32_t N_before_grow;     // cells before this step's grow (link range start)
+    int err;
+    unsigned int ticket;        // last-block election for the sum reduction
+    unsigned long long smax_bits;  // bits of max_c sum_j |u_cj|/h_j  (>= 0, so uint order == fp order)
+    double sumQ;                // sum of stored masses Q
+    double scale;               // P = scale * Q
+    double dt;
+    double dt_cap;              // caller's cap for this step (<= 0 / non-finite: none)
+    double t;
+    double mass;                // pre-normalisation mass of the last step (in normalised units)
+    unsigned long long steps;
+    unsigned long long cell_updates;
+    unsigned int tile_counter;  // dynamic tile ids for the decoupled-lookback scan
+    uint32_t N_after_prune;
+};
+
+struct Pool {
+    uint64_t* key;       // [cap] packed key | KEY_GROWN
+    double* Q;           // [cap] stored mass (P = scale * Q)
+    double* acc;         // [cap] pass-A partial update
+    uint16_t* mask;      // [cap] which face fluxes pass B must gather (bit j: lower, bit 8+j: upper)
+    uint32_t* nbr;       // [2n][cap] adjacency: dir d = 2j (lower, -e^j), 2j+1 (upper, +e^j)
+    double* phi;         // [2n][cap] tau_j * face flux computed by the upwind owner: 2j -> lower face, 2j+1 -> upper face
+    ulonglong2* table;   // [slots] {key, pool index}
+    uint64_t* key2;      // compaction double buffers
+    double* Q2;
+    uint8_t* keep;       // [cap]
+    unsigned long long* tile_state;  // scan descriptors
+    double* partial;     // block partial sums
+};
+
+// ---- key packing (A18): field j at shift (n-1-j)*bits, biased by 2^(bits-1); dim 0 most significant
+__device__ __forceinline__ int field_shift(const Params& p, int j) { return (p.n - 1 - j) * p.bits; }
+
+template <int NDIM>
+__device__ __forceinline__ void unpack(const Params& p, uint64_t key, int32_t c[NDIM]) {
+    const uint64_t m = (1ull << p.bits) - 1ull;
+#pragma unroll
+    for (int j = 0; j < NDIM; ++j)
+        c[j] = (int32_t)((int64_t)((key >> ((NDIM - 1 - j) * p.bits)) & m) - p.bias);
+}
+
+template <int NDIM>
+__device__ __forceinline__ uint64_t pack(const Params& p, const int32_t c[NDIM]) {
+    uint64_t k = 0;
+#pragma unroll
+    for (int j = 0; j < NDIM; ++j) k |= (uint64_t)((int64_t)c[j] + p.bias) << ((NDIM - 1 - j) * p.bits);
+    return k;
+}
+
+// ---- hashtable: open addressing, linear probing, 16-byte slots {key, index} --------------------
+__device__ __forceinline__ uint64_t mix64(uint64_t x) {  // splitmix64 finaliser
+    x ^= x >> 30; x *= 0xbf58476d1ce4e5b9ull;
+    x ^= x >> 27; x *= 0x94d049bb133111ebull;
+    x ^= x >> 31;
+    return x;
+}
+__device__ __forceinline__ uint64_t home_slot(uint64_t key, uint64_t slots) {
+    return __umul64hi(mix64(key), slots);
+}
+
+// returns pool index or NBR_NONE. probes (optional) counts slots inspected.
+__device__ __forceinline__ uint32_t ht_find(const ulonglong2* __restrict__ table, uint64_t slots,
+                                            uint64_t key, unsigned* probes = nullptr) {
+    uint64_t s = home_slot(key, slots);
+    unsigned np = 0;
+    for (;;) {
+        const ulonglong2 e = table[s];
+        ++np;
+        if (e.x == key) { if (probes) *probes += np; return (uint32_t)e.y; }
+        if (e.x == KEY_EMPTY) { if (probes) *probes += np; return NBR_NONE; }
+        if (++s == slots) s = 0;
+    }
+}
+
+// Claim a slot for `key` if absent. Returns the slot index if THIS thread inserted (caller then
+// publishes the value), or ~0ull if the key was already there / the table is full.
+__device__ __forceinline__ uint64_t ht_claim(ulonglong2* table, uint64_t slots, uint64_t key,
+                                             unsigned* probes = nullptr) {
+    uint64_t s = home_slot(key, slots);
+    unsigned np = 0;
+    for (uint64_t tries = 0; tries < slots; ++tries) {
+        unsigned long long* kp = reinterpret_cast<unsigned long long*>(&table[s].x);
+        unsigned long long cur = *reinterpret_cast<volatile unsigned long long*>(kp);
+        ++np;
+        if (cur == KEY_EMPTY) cur = atomicCAS(kp, KEY_EMPTY, key);
+        if (cur == KEY_EMPTY) { if (probes) *probes += np; return s; }
+        if (cur == key) { if (probes) *probes += np; return ~0ull; }
+        if (++s == slots) s = 0;
+    }
+    if (probes) *probes += np;
+    return ~0ull - 1;  // table full
+}
+
+// ---- dynamics (A12): fixed operation order, never fused -------------------------------------
+#define DMUL(a, b) __dmul_rn((a), (b))
+#define DADD(a, b) __dadd_rn((a), (b))
+#define DSUB(a, b) __dsub_rn((a), (b))
+
+// f_j(x) with x[j] replaced by xj (the face coordinate along j)
+template <int NDIM, int DYN>
+__device__ __forceinline__ double dyn_f(const Params& p, const double x[NDIM], int j, double xj) {
+    if constexpr (DYN == 0) {          // Lorenz '63 classic (sigma, beta, rho)
+        if (j == 0) return DMUL(p.par[0], DSUB(x[1], xj));
+        if (j == 1) return DSUB(DMUL(x[0], DSUB(p.par[2], x[2])), xj);
+        return DSUB(DMUL(x[0], x[1]), DMUL(p.par[1], xj));
+    } else if constexpr (DYN == 1) {   // Lorenz '63, PAPER.md:303 (sigma, b, r)
+        if (j == 0) return DMUL(p.par[0], DSUB(x[1], xj));
+        if (j == 1) return DSUB(-xj, DMUL(x[0], x[2]));
+        return DSUB(DSUB(DMUL(x[0], x[1]), DMUL(p.par[1], xj)), DMUL(p.par[1], p.par[2]));
+    } else if constexpr (DYN == 2) {   // Lorenz '96, PAPER.md:319 (cyclic; x_j itself enters only as -x_j)
+        const int jp = (j + 1) % NDIM, jm1 = (j + NDIM - 1) % NDIM, jm2 = (j + NDIM - 2) % NDIM;
+        return DADD(DSUB(DMUL(DSUB(x[jp], x[jm2]), x[jm1]), xj), p.par[0]);
+    } else if constexpr (DYN == 3) {   // linear, ascending m
+        double s = DMUL(p.par[j * NDIM + 0], j == 0 ? xj : x[0]);
+#pragma unroll
+        for (int m = 1; m < NDIM; ++m) s = DADD(s, DMUL(p.par[j * NDIM + m], m == j ? xj : x[m]));
+        return s;
+    } else {                           // constant
+        return p.par[j];
+    }
+}
+
+// cell-centre coordinates and the 2n own face velocities of cell c:
+//   ul[j] = u_{c,j}   (lower j-face),  uu[j] = u_{c+e^j,j} (upper j-face = lower face of c+e^j)
+template <int NDIM, int DYN>
+__device__ __forceinline__ void face_velocities(const Params& p, const int32_t c[NDIM],
+                                                double ul[NDIM], double uu[NDIM]) {
+    double x[NDIM];
+#pragma unroll
+    for (int m = 0; m < NDIM; ++m) x[m] = DADD(p.mu[m], DMUL((double)c[m], p.h[m]));
+#pragma unroll
+    for (int j = 0; j < NDIM; ++j) {
+        const double xl = DADD(p.mu[j], DMUL((double)c[j] - 0.5, p.h[j]));
+        const double xu = DADD(p.mu[j], DMUL((double)c[j] + 0.5, p.h[j]));
+        ul[j] = dyn_f<NDIM, DYN>(p, x, j, xl);
+        uu[j] = dyn_f<NDIM, DYN>(p, x, j, xu);
+    }
+}
+
+// s_c = sum_j |u_{c,j}| / h_j, ascending j, true division (bit-identical to the oracle's Eq. 8 term)
+template <int NDIM>
+__device__ __forceinline__ double cfl_term(const Params& p, const double ul[NDIM]) {
+    double s = 0.0;
+#pragma unroll
+    for (int j = 0; j < NDIM; ++j) s = DADD(s, __ddiv_rn(fabs(ul[j]), p.h[j]));
+    return s;
+}
+
+// monotonised-central limiter, division-free (A3)
+__device__ __forceinline__ double mc_limit(double a, double b) {
+    if (a * b <= 0.0) return 0.0;
+    const double m = fmin(0.5 * fabs(a + b), fmin(2.0 * fabs(a), 2.0 * fabs(b)));
+    return a > 0.0 ? m : -m;
+}
+
+}  // namespace gbees

@@ -1,0 +1,544 @@
+// Kernels of the GBEES prediction step. Every phase is a grid-stride __device__ function so the
+// same code runs as a stream of small launches (gbees_step) or inside the persistent cooperative
+// loop (gbees_run). Semantics: DESIGN.md D1-D5; layout: DESIGN.md "Data layout".
+#pragma once
+#include "gbees_common.cuh"
+
+namespace gbees {
+
+constexpr int TPB = 256;
+
+__device__ __forceinline__ unsigned gtid() { return blockIdx.x * blockDim.x + threadIdx.x; }
+__device__ __forceinline__ unsigned gthreads() { return gridDim.x * blockDim.x; }
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ double warp_max(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+// block-wide sum, result valid in thread 0. Fixed order => deterministic for a fixed launch shape.
+__device__ __forceinline__ double block_sum(double v) {
+    __shared__ double sh[32];
+    __syncthreads();
+    v = warp_sum(v);
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double r = 0.0;
+    if (threadIdx.x < 32) {
+        r = threadIdx.x < (blockDim.x >> 5) ? sh[threadIdx.x] : 0.0;
+        r = warp_sum(r);
+    }
+    return r;
+}
+__device__ __forceinline__ double block_max(double v) {
+    __shared__ double shm[32];
+    __syncthreads();
+    v = warp_max(v);
+    if ((threadIdx.x & 31) == 0) shm[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double r = 0.0;
+    if (threadIdx.x < 32) {
+        r = threadIdx.x < (blockDim.x >> 5) ? shm[threadIdx.x] : 0.0;
+        r = warp_max(r);
+    }
+    return r;
+}
+
+// ---- Targets(c), D1.1 / A10 / A11: downwind face + pairwise-edge neighbours -------------------
+// fn(key, in_range). Range: a coordinate must stay inside the packable field.
+template <int NDIM, typename F>
+__device__ __forceinline__ void for_each_target(const Params& p, uint64_t key, const int32_t c[NDIM],
+                                                const double ul[NDIM], const double uu[NDIM], F&& fn) {
+    const int32_t lo = (int32_t)(-p.bias), hi = (int32_t)(p.bias - 1);
+    // per dim: bit0 = outflow through lower face (u<0), bit1 = outflow through upper face (u>0)
+    int o[NDIM];
+#pragma unroll
+    for (int j = 0; j < NDIM; ++j) o[j] = (ul[j] < 0.0 ? 1 : 0) | (uu[j] > 0.0 ? 2 : 0);
+#pragma unroll
+    for (int j = 0; j < NDIM; ++j) {
+        const uint64_t uj = 1ull << ((NDIM - 1 - j) * p.bits);
+#pragma unroll
+        for (int sj = 0; sj < 2; ++sj) {
+            if (!(o[j] & (1 << sj))) continue;
+            const bool okj = sj ? (c[j] < hi) : (c[j] > lo);
+            const uint64_t kj = sj ? key + uj : key - uj;
+            fn(kj, okj);
+#pragma unroll
+            for (int l = j + 1; l < NDIM; ++l) {
+                const uint64_t ulk = 1ull << ((NDIM - 1 - l) * p.bits);
+#pragma unroll
+                for (int sl = 0; sl < 2; ++sl) {
+                    if (!(o[l] & (1 << sl))) continue;
+                    const bool okl = sl ? (c[l] < hi) : (c[l] > lo);
+                    fn(sl ? kj + ulk : kj - ulk, okj && okl);
+                }
+            }
+        }
+    }
+}
+
+// ---- a1 grow (Alg. 2 without staging: atomicCAS claims the slot) ------
+template <int NDIM, int DYN>
+__device__ void phase_grow(const Params& p, const Pool& pool, DevState* st) {
+    const uint32_t N0 = st->N_before_grow;
+    const double scale = st->scale;
+    for (uint32_t i = gtid(); i < N0; i += gthreads()) {
+        const uint64_t kf = pool.key[i];
+        if (kf & KEY_GROWN) continue;                 // targets already inserted (autonomous f)
+        if (!(scale * pool.Q[i] >= p.thresh)) continue;
+        int32_t c[NDIM];
+        unpack<NDIM>(p, kf, c);
+        double ul[NDIM], uu[NDIM];
+        face_velocities<NDIM, DYN>(p, c, ul, uu);
+        for_each_target<NDIM>(p, kf, c, ul, uu, [&](uint64_t tk, bool ok) {
+            if (!ok) { atomicOr(&st->err, E_KEY_RANGE); return; }
+            const uint64_t s = ht_claim(pool.table, p.slots, tk);
+            if (s == ~0ull) return;                   // already there
+            if (s == ~0ull - 1) { atomicOr(&st->err, E_TABLE_FULL); return; }
+            const uint32_t idx = atomicAdd(&st->N, 1u);
+            if (idx >= p.cap) { atomicOr(&st->err, E_CAPACITY); pool.table[s].y = NBR_NONE; return; }
+            pool.table[s].y = idx;
+            pool.key[idx] = tk;
+            pool.Q[idx] = 0.0;
+#pragma unroll
+            for (int d = 0; d < 2 * NDIM; ++d) pool.nbr[(size_t)d * p.cap + idx] = NBR_NONE;
+        });
+        pool.key[i] = kf | KEY_GROWN;
+    }
+}
+
+// ---- adjacency + CFL term of the linked cells -----------------------------------
+// ALL = true: rebuild for every cell (after init / import / prune); false: only cells created by
+// this step's grow, which also patch the slots of their neighbours. atomicMin makes a direct
+// index (< NBR_TAG) win over a tagged two-hop index, which wins over NBR_NONE.
+template <int NDIM, int DYN, bool ALL>
+__device__ void phase_link(const Params& p, const Pool& pool, DevState* st) {
+    const uint32_t first = ALL ? 0u : st->N_before_grow;
+    const uint32_t N = min(st->N, p.cap);
+    const int32_t lo = (int32_t)(-p.bias), hi = (int32_t)(p.bias - 1);
+    double smax = 0.0;
+    for (uint32_t i = first + gtid(); i < N; i += gthreads()) {
+        const uint64_t key = pool.key[i] & ~KEY_GROWN;
+        int32_t c[NDIM];
+        unpack<NDIM>(p, key, c);
+#pragma unroll
+        for (int j = 0; j < NDIM; ++j) {
+            const uint64_t uj = 1ull << ((NDIM - 1 - j) * p.bits);
+#pragma unroll
+            for (int s = 0; s < 2; ++s) {
+                const int d = 2 * j + s, od = 2 * j + (1 - s);
+                uint32_t* mine = &pool.nbr[(size_t)d * p.cap + i];
+                uint32_t val = NBR_NONE;
+                const bool ok1 = s ? (c[j] < hi) : (c[j] > lo);
+                if (ok1) {
+                    const uint32_t nb = ht_find(pool.table, p.slots, s ? key + uj : key - uj);
+                    if (nb != NBR_NONE) {
+                        val = nb;
+                        if (!ALL) atomicMin(&pool.nbr[(size_t)od * p.cap + nb], i);
+                    } else if (s ? (c[j] < hi - 1) : (c[j] > lo + 1)) {
+                        const uint32_t nb2 = ht_find(pool.table, p.slots, s ? key + 2 * uj : key - 2 * uj);
+                        if (nb2 != NBR_NONE) {
+                            val = NBR_TAG | nb2;
+                            if (!ALL) atomicMin(&pool.nbr[(size_t)od * p.cap + nb2], NBR_TAG | i);
+                        }
+                    }
+                }
+                if (ALL) *mine = val;
+                else if (val != NBR_NONE) atomicMin(mine, val);
+            }
+        }
+        double ul[NDIM], uu[NDIM];
+        face_velocities<NDIM, DYN>(p, c, ul, uu);
+        smax = fmax(smax, cfl_term<NDIM>(p, ul));
+    }
+    smax = block_max(smax);
+    if (threadIdx.x == 0 && smax > 0.0) atomicMax(&st->smax_bits, (unsigned long long)__double_as_longlong(smax));
+}
+
+// dt of Eq. (8) with the caller's cap (every thread computes the same value)
+__device__ __forceinline__ double step_dt(const Params& p, const DevState* st) {
+    const double smax = __longlong_as_double((long long)st->smax_bits);
+    const double cap = st->dt_cap;
+    const bool capped = isfinite(cap) && cap > 0.0;
+    double dt = smax > 0.0 ? __ddiv_rn(p.cfl, smax) : (capped ? cap : 0.0);
+    if (capped && cap < dt) dt = cap;
+    return dt;
+}
+
+// ---- a2+a4 pass A: every active cell computes the fluxes of the faces it is UPWIND of -----------
+// Gather form D2 (= Eq. 7 + Alg. 1 + high-resolution term):
+//   T_l   = u+_{c,l}(P_c - P_{c-e^l}) + u-_{c+e^l,l}(P_{c+e^l} - P_c)
+//   G_j   = P*_{c,(j)} = P_c - sum_{l != j} 1/2 tau_l T_l
+//   sig_j = mc(P_c - P_{c-e^j}, P_{c+e^j} - P_c)     (limited wave when c is the upwind cell)
+//   upper face, u = u_{c+e^j,j} > 0:  F = u (G_j + 1/2 (1 - tau_j u) sig_j)
+//   lower face, u = u_{c,j}     < 0:  F = u (G_j - 1/2 (1 + tau_j u) sig_j)
+// A face whose upwind cell is NOT active carries only the high-resolution term; the active
+// downwind cell computes it (needs the two-hop value through the tagged adjacency slot).
+// acc_c = P_c - sum_j tau_j (F_up - F_lo) over the faces computed here; tau_j F is stored for the
+// neighbour that shares the face; mask tells pass B which faces to fetch from neighbours.
+template <int NDIM, int DYN>
+__device__ void phase_passA(const Params& p, const Pool& pool, DevState* st) {
+    const uint32_t N = min(st->N, p.cap);
+    const double dt = step_dt(p, st);
+    double tau[NDIM];
+#pragma unroll
+    for (int j = 0; j < NDIM; ++j) tau[j] = dt / p.h[j];
+    const size_t cap = p.cap;
+    for (uint32_t i = gtid(); i < N; i += gthreads()) {
+        const uint64_t key = pool.key[i] & ~KEY_GROWN;
+        int32_t c[NDIM];
+        unpack<NDIM>(p, key, c);
+        const double q0 = pool.Q[i];
+        double qm[NDIM], qp[NDIM], qmm[NDIM], qpp[NDIM];
+        bool hasm[NDIM], hasp[NDIM];
+#pragma unroll
+        for (int j = 0; j < NDIM; ++j) {
+            const uint32_t nm = pool.nbr[(size_t)(2 * j) * cap + i];
+            const uint32_t np = pool.nbr[(size_t)(2 * j + 1) * cap + i];
+            hasm[j] = nm < NBR_TAG;
+            hasp[j] = np < NBR_TAG;
+            const double vm = nm != NBR_NONE ? pool.Q[nm & ~NBR_TAG] : 0.0;
+            const double vp = np != NBR_NONE ? pool.Q[np & ~NBR_TAG] : 0.0;
+            qm[j] = hasm[j] ? vm : 0.0;  qmm[j] = hasm[j] ? 0.0 : vm;
+            qp[j] = hasp[j] ? vp : 0.0;  qpp[j] = hasp[j] ? 0.0 : vp;
+        }
+        double ul[NDIM], uu[NDIM];
+        face_velocities<NDIM, DYN>(p, c, ul, uu);
+        double T[NDIM];
+#pragma unroll
+        for (int l = 0; l < NDIM; ++l)
+            T[l] = 0.5 * tau[l] * (fmax(ul[l], 0.0) * (q0 - qm[l]) + fmin(uu[l], 0.0) * (qp[l] - q0));
+        double acc = q0;
+        unsigned mask = 0;
+#pragma unroll
+        for (int j = 0; j < NDIM; ++j) {
+            double G = q0;
+#pragma unroll
+            for (int l = 0; l < NDIM; ++l)
+                if (l != j) G -= T[l];
+            const double dm = q0 - qm[j], dp = qp[j] - q0;
+            const double sig = p.hi_res ? (p.limiter ? 0.0 : mc_limit(dm, dp)) : 0.0;
+            {   // upper face of c
+                const double u = uu[j];
+                if (u > 0.0) {
+                    const double w = p.hi_res ? (p.limiter ? dp : sig) : 0.0;
+                    const double F = tau[j] * (u * G + 0.5 * u * (1.0 - tau[j] * u) * w);
+                    acc -= F;
+                    if (hasp[j]) pool.phi[(size_t)(2 * j + 1) * cap + i] = F;
+                } else if (u < 0.0) {
+                    if (hasp[j]) {
+                        mask |= 1u << (8 + j);
+                    } else if (p.hi_res) {   // upwind cell c+e^j inactive: W = 0 - P_c, W_up = P_{c+2e^j} - 0
+                        const double w = p.limiter ? -q0 : mc_limit(-q0, qpp[j]);
+                        acc -= tau[j] * (0.5 * (-u) * (1.0 + tau[j] * u) * w);
+                    }
+                }
+            }
+            {   // lower face of c
+                const double u = ul[j];
+                if (u < 0.0) {
+                    const double w = p.hi_res ? (p.limiter ? dm : sig) : 0.0;
+                    const double F = tau[j] * (u * G + 0.5 * (-u) * (1.0 + tau[j] * u) * w);
+                    acc += F;
+                    if (hasm[j]) pool.phi[(size_t)(2 * j) * cap + i] = F;
+                } else if (u > 0.0) {
+                    if (hasm[j]) {
+                        mask |= 1u << j;
+                    } else if (p.hi_res) {   // upwind cell c-e^j inactive: W = P_c - 0, W_up = 0 - P_{c-2e^j}
+                        const double w = p.limiter ? q0 : mc_limit(q0, -qmm[j]);
+                        acc += tau[j] * (0.5 * u * (1.0 - tau[j] * u) * w);
+                    }
+                }
+            }
+        }
+        pool.acc[i] = acc;
+        pool.mask[i] = (uint16_t)mask;
+    }
+}
+
+// ---- a5+a6 pass B: fetch the fluxes owned by neighbours, finish the update, sum the mass --------
+template <int NDIM>
+__device__ void phase_passB(const Params& p, const Pool& pool, DevState* st) {
+    const uint32_t N = min(st->N, p.cap);
+    const size_t cap = p.cap;
+    double sum = 0.0;
+    for (uint32_t i = gtid(); i < N; i += gthreads()) {
+        double a = pool.acc[i];
+        const unsigned mask = pool.mask[i];
+#pragma unroll
+        for (int j = 0; j < NDIM; ++j) {
+            if (mask & (1u << j)) {          // lower face: flux computed by c-e^j as its upper face
+                const uint32_t b = pool.nbr[(size_t)(2 * j) * cap + i];
+                a += pool.phi[(size_t)(2 * j + 1) * cap + b];
+            }
+            if (mask & (1u << (8 + j))) {    // upper face: flux computed by c+e^j as its lower face
+                const uint32_t b = pool.nbr[(size_t)(2 * j + 1) * cap + i];
+                a -= pool.phi[(size_t)(2 * j) * cap + b];
+            }
+        }
+        pool.Q[i] = a;
+        sum += a;
+    }
+    sum = block_sum(sum);
+    if (threadIdx.x == 0) pool.partial[blockIdx.x] = sum;
+}
+
+// plain sum of Q (init / correct / prune); same partial[] protocol as pass B
+__device__ void phase_sum(const Params& p, const Pool& pool, DevState* st) {
+    const uint32_t N = min(st->N, p.cap);
+    double sum = 0.0;
+    for (uint32_t i = gtid(); i < N; i += gthreads()) sum += pool.Q[i];
+    sum = block_sum(sum);
+    if (threadIdx.x == 0) pool.partial[blockIdx.x] = sum;
+}
+
+// one block: add the partials in index order, set the scale. after_step: advance t, count.
+__device__ void finish_sum(const Params& p, const Pool& pool, DevState* st, unsigned nparts, bool after_step) {
+    double v = 0.0;
+    for (unsigned k = threadIdx.x; k < nparts; k += blockDim.x) v += pool.partial[k];
+    v = block_sum(v);
+    if (threadIdx.x == 0) {
+        st->sumQ = v;
+        if (!(v > 0.0) || !isfinite(v)) {
+            if (p.normalise || !isfinite(v)) atomicOr(&st->err, E_DEGENERATE);
+        }
+        const double old = st->scale;
+        st->mass = v * old;
+        if (p.normalise && v > 0.0) st->scale = 1.0 / v;
+        if (after_step) {
+            const double dt = step_dt(p, st);
+            if (!(dt > 0.0)) atomicOr(&st->err, E_DEGENERATE);
+            st->dt = dt;
+            st->t += dt;
+            st->steps += 1;
+            st->cell_updates += min(st->N, p.cap);
+        }
+    }
+}
+
+}  // namespace gbees
+
+namespace gbees {
+
+// ---- a7 prune, D3 (Alg. 3) -------------------------------------------
+// mark: keep c if P_c >= p*, and keep every existing grow-target of such a cell.
+template <int NDIM, int DYN>
+__device__ void phase_mark(const Params& p, const Pool& pool, DevState* st) {
+    const uint32_t N = min(st->N, p.cap);
+    const double scale = st->scale;
+    for (uint32_t i = gtid(); i < N; i += gthreads()) {
+        const uint64_t kf = pool.key[i];
+        if (!(scale * pool.Q[i] >= p.thresh)) continue;
+        pool.keep[i] = 1;
+        const uint64_t key = kf & ~KEY_GROWN;
+        int32_t c[NDIM];
+        unpack<NDIM>(p, key, c);
+        double ul[NDIM], uu[NDIM];
+        face_velocities<NDIM, DYN>(p, c, ul, uu);
+        for_each_target<NDIM>(p, key, c, ul, uu, [&](uint64_t tk, bool ok) {
+            if (!ok) return;
+            const uint32_t nb = ht_find(pool.table, p.slots, tk);
+            if (nb != NBR_NONE) pool.keep[nb] = 1;
+        });
+    }
+}
+
+// Single-pass stream compaction with a decoupled-lookback scan over tiles of SCAN_TILE flags.
+// tile_state[t] = (status << 32) | value, status 0 = invalid, 1 = aggregate, 2 = inclusive prefix.
+// Tiles are handed out by an atomic counter so a tile's predecessors are always running or done.
+constexpr int SCAN_ITEMS = 8;
+constexpr int SCAN_TILE = TPB * SCAN_ITEMS;
+
+// Generic core: flags -> stable destination index; body(i, dst) is called for kept items.
+template <typename KeepFn, typename MoveFn>
+__device__ void scan_compact(uint32_t N, unsigned long long* tile_state, unsigned int* tile_counter,
+                             uint32_t* total_out, KeepFn keepf, MoveFn movef) {
+    __shared__ unsigned s_tile;
+    __shared__ uint32_t s_warp[TPB / 32];
+    __shared__ uint32_t s_prefix;
+    const unsigned ntiles = (N + SCAN_TILE - 1) / SCAN_TILE;
+    for (;;) {
+        __syncthreads();
+        if (threadIdx.x == 0) s_tile = atomicAdd(tile_counter, 1u);
+        __syncthreads();
+        const unsigned tile = s_tile;
+        if (tile >= ntiles) break;
+        const uint32_t base = tile * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
+        uint32_t f[SCAN_ITEMS], local = 0;
+#pragma unroll
+        for (int k = 0; k < SCAN_ITEMS; ++k) {
+            f[k] = (base + k < N && keepf(base + k)) ? 1u : 0u;
+            local += f[k];
+        }
+        // block exclusive scan of `local`
+        uint32_t incl = local;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
+            if ((threadIdx.x & 31) >= o) incl += v;
+        }
+        if ((threadIdx.x & 31) == 31) s_warp[threadIdx.x >> 5] = incl;
+        __syncthreads();
+        uint32_t woff = 0, tile_total = 0;
+#pragma unroll
+        for (int w = 0; w < TPB / 32; ++w) {
+            if (w < (int)(threadIdx.x >> 5)) woff += s_warp[w];
+            tile_total += s_warp[w];
+        }
+        // publish aggregate, look back
+        if (threadIdx.x == 0) {
+            if (tile == 0) {
+                atomicExch(&tile_state[0], (2ull << 32) | tile_total);
+                s_prefix = 0;
+            } else {
+                atomicExch(&tile_state[tile], (1ull << 32) | tile_total);
+                uint32_t run = 0;
+                for (int t = (int)tile - 1;; --t) {
+                    unsigned long long v;
+                    do { v = *reinterpret_cast<volatile unsigned long long*>(&tile_state[t]); } while ((v >> 32) == 0);
+                    run += (uint32_t)v;
+                    if ((v >> 32) == 2) break;
+                }
+                atomicExch(&tile_state[tile], (2ull << 32) | (run + tile_total));
+                s_prefix = run;
+            }
+            if (tile == ntiles - 1) *total_out = s_prefix + tile_total;
+        }
+        __syncthreads();
+        uint32_t dst = s_prefix + woff + (incl - local);
+#pragma unroll
+        for (int k = 0; k < SCAN_ITEMS; ++k)
+            if (f[k]) movef(base + k, dst++);
+    }
+}
+
+__device__ void phase_compact(const Params& p, const Pool& pool, DevState* st) {
+    const uint32_t N = min(st->N, p.cap);
+    const double scale = st->scale;
+    const double thresh = p.thresh;
+    if (N == 0) { if (gtid() == 0) st->N_after_prune = 0; return; }
+    scan_compact(
+        N, pool.tile_state, &st->tile_counter, &st->N_after_prune,
+        [&](uint32_t i) { return pool.keep[i] != 0; },
+        [&](uint32_t i, uint32_t d) {
+            const uint64_t kf = pool.key[i];
+            const double q = pool.Q[i];
+            // the GROWN flag survives only for cells still >= p* (their targets were all kept)
+            pool.key2[d] = (scale * q >= thresh) ? kf : (kf & ~KEY_GROWN);
+            pool.Q2[d] = q;
+        });
+}
+
+// after the pointer swap: insert every pool key with its row index (table was cleared)
+__device__ void phase_rebuild(const Params& p, const Pool& pool, DevState* st) {
+    const uint32_t N = min(st->N, p.cap);
+    for (uint32_t i = gtid(); i < N; i += gthreads()) {
+        const uint64_t key = pool.key[i] & ~KEY_GROWN;
+        const uint64_t s = ht_claim(pool.table, p.slots, key);
+        if (s >= ~0ull - 1) { atomicOr(&st->err, s == ~0ull ? E_DEGENERATE : E_TABLE_FULL); continue; }  // duplicate key
+        pool.table[s].y = i;
+    }
+}
+
+// ---- D5 / A8 init_gaussian: one thread per candidate cell of the ellipsoid's bounding box ---------
+struct GaussArgs {
+    double inv[MAXN * MAXN];   // Sigma^-1 (or R^-1 for correct)
+    double v[MAXN];            // correct: measurement z
+    double norm;               // P~ at the mean
+    int64_t R[MAXN];           // half-extents of the bounding box in cells
+    unsigned long long total;  // prod (2 R_j + 1)
+};
+
+template <int NDIM>
+__device__ __forceinline__ double quad_form(const double* inv, const double d[NDIM]) {
+    double q = 0.0;
+#pragma unroll
+    for (int i = 0; i < NDIM; ++i) {
+        double r = 0.0;
+#pragma unroll
+        for (int j = 0; j < NDIM; ++j) r += inv[i * NDIM + j] * d[j];
+        q += d[i] * r;
+    }
+    return q;
+}
+
+template <int NDIM>
+__device__ void phase_init_gaussian(const Params& p, const Pool& pool, DevState* st, const GaussArgs& g) {
+    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+    for (unsigned long long r = gtid(); r < g.total; r += stride) {
+        int32_t c[NDIM];
+        unsigned long long rem = r;
+#pragma unroll
+        for (int j = NDIM - 1; j >= 0; --j) {
+            const unsigned long long w = 2ull * g.R[j] + 1ull;
+            c[j] = (int32_t)((long long)(rem % w) - g.R[j]);
+            rem /= w;
+        }
+        double d[NDIM];
+#pragma unroll
+        for (int j = 0; j < NDIM; ++j) d[j] = (double)c[j] * p.h[j];
+        const double val = exp(-0.5 * quad_form<NDIM>(g.inv, d)) * g.norm;
+        if (!(val >= p.thresh)) continue;
+        bool ok = true;
+#pragma unroll
+        for (int j = 0; j < NDIM; ++j) ok = ok && c[j] >= -p.bias && c[j] <= p.bias - 1;
+        if (!ok) { atomicOr(&st->err, E_KEY_RANGE); continue; }
+        const uint32_t idx = atomicAdd(&st->N, 1u);
+        if (idx >= p.cap) { atomicOr(&st->err, E_CAPACITY); continue; }
+        pool.key[idx] = pack<NDIM>(p, c);
+        pool.Q[idx] = val;
+    }
+}
+
+// ---- a8 correct, D4 / Eq. (4): Q_c *= exp(-1/2 (z - x_c)^T R^-1 (z - x_c)) ------------
+template <int NDIM>
+__device__ void phase_correct(const Params& p, const Pool& pool, DevState* st, const GaussArgs& g) {
+    const uint32_t N = min(st->N, p.cap);
+    for (uint32_t i = gtid(); i < N; i += gthreads()) {
+        int32_t c[NDIM];
+        unpack<NDIM>(p, pool.key[i] & ~KEY_GROWN, c);
+        double d[NDIM];
+#pragma unroll
+        for (int j = 0; j < NDIM; ++j) d[j] = g.v[j] - (p.mu[j] + (double)c[j] * p.h[j]);
+        pool.Q[i] *= exp(-0.5 * quad_form<NDIM>(g.inv, d));
+    }
+}
+
+template <int NDIM>
+__device__ void phase_export(const Params& p, const Pool& pool, const DevState* st, int32_t* keys, double* out) {
+    const uint32_t N = min(st->N, p.cap);
+    const double scale = st->scale;
+    for (uint32_t i = gtid(); i < N; i += gthreads()) {
+        if (keys) {
+            int32_t c[NDIM];
+            unpack<NDIM>(p, pool.key[i] & ~KEY_GROWN, c);
+#pragma unroll
+            for (int j = 0; j < NDIM; ++j) keys[(size_t)i * NDIM + j] = c[j];
+        }
+        if (out) out[i] = scale * pool.Q[i];
+    }
+}
+
+template <int NDIM>
+__device__ void phase_import(const Params& p, const Pool& pool, DevState* st, const int32_t* keys,
+                             const double* vals, uint32_t count) {
+    for (uint32_t i = gtid(); i < count; i += gthreads()) {
+        int32_t c[NDIM];
+        bool ok = true;
+#pragma unroll
+        for (int j = 0; j < NDIM; ++j) {
+            c[j] = keys[(size_t)i * NDIM + j];
+            ok = ok && c[j] >= -p.bias && c[j] <= p.bias - 1;
+        }
+        if (!ok) { atomicOr(&st->err, E_KEY_RANGE); for (int j = 0; j < NDIM; ++j) c[j] = 0; }
+        pool.key[i] = pack<NDIM>(p, c);
+        pool.Q[i] = vals[i];
+    }
+}
+
+}  // namespace gbees

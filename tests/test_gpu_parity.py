@@ -1,0 +1,160 @@
+"""GPU-vs-oracle parity through the C ABI (python binding = argument marshalling only)."""
+import itertools
+
+import numpy as np
+import pytest
+
+from oracle.binding import Oracle
+from paper_2508_13986_b200 import workloads as W
+from util import compare_states
+
+pytestmark = pytest.mark.gpu
+
+
+def G(*a, **k):
+    from paper_2508_13986_b200 import Gbees
+    return Gbees(*a, **k)
+
+
+def box(lo, hi):
+    return np.array(list(itertools.product(*[range(a, b) for a, b in zip(lo, hi)])), dtype=np.int32)
+
+
+def pair_raw(n, h, dyn, params, keys, p, origin, hi_res=1, limiter=0, cfl=0.9):
+    o = Oracle(n, h, 1e-300, dyn, params, cfl=cfl, hi_res=hi_res, limiter=limiter)
+    o.set_flags(grow=False, normalise=False)
+    o.import_state(origin, keys, p)
+    g = G(n, h, 1e-300, dyn, params, cfl=cfl, hi_res=hi_res, limiter=limiter, no_grow=True, no_normalise=True,
+          max_cells=1 << 16)
+    g.import_state(origin, keys, p)
+    return g, o
+
+
+@pytest.mark.parametrize("n,axis,sign", [(1, 0, 1), (3, 1, 1), (3, 2, -1), (6, 4, 1), (6, 0, -1)])
+def test_courant_one_shift_bit_exact(n, axis, sign):
+    rng = np.random.default_rng(W.S0 + 202)
+    v = np.zeros(n); v[axis] = 2.0 * sign
+    hi = [3] * n; hi[axis] = 12
+    keys = box([0] * n, hi)
+    p = rng.integers(0, 64, len(keys)).astype(np.float64) * 2.0 ** -9
+    p[(keys[:, axis] < 2) | (keys[:, axis] >= 10)] = 0.0
+    for hi_res, limiter in [(0, 0), (1, 0), (1, 1)]:
+        g, o = pair_raw(n, [0.5] * n, 4, v, keys, p, np.zeros(n), hi_res, limiter, cfl=1.0)
+        assert g.step() == o.step() == 0.25
+        gk, gp = g.export(); ok, op = o.export()
+        assert np.array_equal(gk, ok) and np.array_equal(gp, op)
+
+
+CASES = [
+    (3, 6, 0, [10, 8 / 3, 28], [-11.5, -10, 9.5]),
+    (3, 9, 1, [4.0, 1.0, 48.0], [-11.5, -10, 9.5]),
+    (4, 5, 2, [4.0], [4.01, 4, 4, 4]),
+    (5, 4, 2, [4.0], [4.01, 4, 4, 4, 4]),
+    (6, 4, 2, [4.0], [4.01, 4, 4, 4, 4, 4]),
+    (6, 3, 3, None, [0.3, -0.2, 0.1, 0.5, -0.4, 0.2]),
+    (2, 20, 3, None, [0.3, -0.2]),
+    (1, 50, 3, [-0.7], [0.3]),
+]
+
+
+@pytest.mark.parametrize("n,side,dyn,params,origin", CASES)
+@pytest.mark.parametrize("ragged", [False, True])
+def test_frozen_grid_flux_update(n, side, dyn, params, origin, ragged):
+    """a2-a6 on a frozen grid (no grow, no normalise): random masses incl. negatives, ragged sets."""
+    rng = np.random.default_rng(W.S0 + 207 + 10 * n + dyn + ragged)
+    if params is None:
+        params = rng.normal(0, 0.3, (n, n)).ravel()
+    h = rng.uniform(0.3, 0.6, n)
+    keys = box([-(side // 2)] * n, [side - side // 2] * n)
+    if ragged:
+        keys = keys[rng.random(len(keys)) < 0.6]
+    p = rng.random(len(keys)) - 0.1
+    for hi_res, limiter in [(0, 0), (1, 0), (1, 1)]:
+        g, o = pair_raw(n, h, dyn, params, keys, p, origin, hi_res, limiter)
+        for _ in range(3):
+            dg, do = g.step(), o.step()
+            assert dg == do                                   # dt bit-identical (A12)
+            gk, gp = g.export(); ok, op = o.export()
+            assert np.array_equal(gk, ok)
+            assert np.max(np.abs(gp - op)) <= 1e-12 * np.max(np.abs(op))
+            assert g.last_mass() == pytest.approx(o.last_mass(), rel=1e-12)
+
+
+def run_lockstep(cfg, steps, check_every=1, rtol_step=1e-10):
+    o = Oracle(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfg["cfl"])
+    g = G(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfg["cfl"], max_cells=cfg["max_cells"])
+    o.init_gaussian(cfg["mean"], cfg["cov"]); g.init_gaussian(cfg["mean"], cfg["cov"])
+    compare_states(*g.export(), *o.export(), cfg["thresh"], 1e-13, what="init")
+    worst = 0.0
+    for k in range(1, steps + 1):
+        dg, do = g.step(), o.step()
+        assert abs(dg - do) <= 1e-14 * do, f"dt mismatch at step {k}: {dg} vs {do}"
+        if cfg["prune_every"] and k % cfg["prune_every"] == 0:
+            g.prune(); o.prune()
+        if k % check_every == 0 or k == steps:
+            assert g.count() == o.count(), f"step {k}: {g.count()} vs {o.count()} cells"
+            worst = max(worst, compare_states(*g.export(), *o.export(), cfg["thresh"], rtol_step, what=f"step {k}"))
+            assert g.time() == pytest.approx(o.time(), rel=1e-14)
+    return worst, g, o
+
+
+def test_config0_lockstep_20_steps():
+    worst, g, o = run_lockstep(W.config0(), 20)
+    assert worst <= 1e-10
+    assert g.stats()["steps"] == 20
+
+
+def test_lorenz96_6d_small_lockstep():
+    cfg = W.config2()
+    cfg.update(thresh=1e-5, max_cells=1 << 20)   # same physics, fewer cells: oracle finishes in seconds
+    worst, g, o = run_lockstep(cfg, 7)
+    assert worst <= 1e-10
+
+
+def test_config1_short_with_corrections():
+    cfg = W.config1()
+    cfg.update(dx=[0.5] * 3)
+    o = Oracle(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfg["cfl"])
+    g = G(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfg["cfl"], max_cells=1 << 18)
+    o.init_gaussian(cfg["mean"], cfg["cov"]); g.init_gaussian(cfg["mean"], cfg["cov"])
+    for tm, z in zip([0.02, 0.04], cfg["z"]):
+        k = 0
+        while o.time() < tm:
+            dg, do = g.step(tm - g.time()), o.step(tm - o.time())
+            assert abs(dg - do) <= 1e-14 * do
+            g.prune(); o.prune()
+            k += 1
+        assert g.time() == o.time() == tm
+        # measurement near the current blob so the posterior keeps mass on the grid
+        kk, pp = o.export()
+        zc = np.array(cfg["mean"]) + (pp[:, None] * kk).sum(0) * np.array(cfg["dx"]) + 0.3
+        g.correct(zc, cfg["R"]); o.correct(zc, cfg["R"])
+        g.prune(); o.prune()
+        compare_states(*g.export(), *o.export(), cfg["thresh"], 1e-10, what=f"after correct t={tm}")
+
+
+def test_errors_and_edges():
+    from paper_2508_13986_b200 import GbeesError
+    g = G(3, [0.5] * 3, 2e-5, 0, [10, 8 / 3, 28], max_cells=1000)
+    with pytest.raises(GbeesError) as e:
+        g.init_gaussian([-11.5, -10, 9.5], np.eye(3))   # needs 1357 cells
+    assert e.value.code == -4
+    g = G(3, [0.5] * 3, 2e-5, 0, [10, 8 / 3, 28], max_cells=4096)
+    with pytest.raises(GbeesError) as e:
+        g.init_gaussian([0, 0, 0], np.array([[1, 2, 0], [2, 1, 0], [0, 0, 1.0]]))
+    assert e.value.code == -3
+    with pytest.raises(GbeesError) as e:
+        g.step()                                           # empty grid
+    assert e.value.code == -6
+    # key range: 6-D fields hold [-512, 511]
+    g = G(6, [0.5] * 6, 1e-3, 4, [1.0] * 6, max_cells=4096)
+    g.import_state(np.zeros(6), np.array([[511, 0, 0, 0, 0, 0]], dtype=np.int32), np.array([1.0]))
+    with pytest.raises(GbeesError) as e:
+        g.step()
+    assert e.value.code == -7
+    # single cell, constant velocity: grows its downwind face/edge neighbours, mass stays 1
+    g = G(3, [0.5] * 3, 1e-3, 4, [1.0, -1.0, 0.0], max_cells=4096)
+    g.import_state(np.zeros(3), np.zeros((1, 3), dtype=np.int32), np.array([1.0]))
+    g.step()
+    k, p = g.export()
+    assert len(k) == 4 and p.sum() == pytest.approx(1.0, abs=1e-15)
