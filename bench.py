@@ -1,0 +1,275 @@
+#!/usr/bin/env python
+"""bench.py -- active-cell CTU updates/s of the GBEES prediction step on B200 (BASELINE.json metric).
+
+A bench "step" = one complete propagation job of the workload (default: BASELINE config 2, the
+6-D Lorenz '96 headline: init -> t = 0.5, CFL 0.9, prune every 5 steps), i.e. one pass of the whole
+hot path (grow, dt, CTU flux, update, normalise, prune/compact/rehash) over one synthetic input.
+`value` = sum over integration steps of the active-cell count / device time of the jobs
+(init_gaussian and export outside the timed region); `e2e` = the same jobs timed through the C ABI
+with HOST buffers: init_gaussian(host mean/cov) + run + export into pinned host arrays.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg2|cfg3|cfg3s|cfg0|cfg1] [--impl reference]
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "active-cell CTU updates/sec (grow+flux+update+prune) at 6-D"
+UNIT = "cell-updates/s"
+
+
+def workload(name):
+    from paper_2508_13986_b200 import workloads as W
+    if name == "cfg0":
+        return W.config0()
+    if name == "cfg1":
+        return W.config1()
+    if name == "cfg2":
+        return W.config2()
+    if name == "cfg3":
+        return W.config3()
+    if name == "cfg3s":  # 1/10-scale twin of config 3
+        c = W.config3(dx=0.5)
+        c.update(name="cfg3_linear_6d_tenth_scale", max_cells=1 << 25)
+        return c
+    raise SystemExit(f"unknown workload {name}")
+
+
+def algo_bytes(stats, n, alpha):
+    """Algorithmic bytes of a job, SURVEY.md 8(d) / DESIGN.md: N*(40+8n) + N_new*(28+8n) + N_prune*(45+8/alpha)."""
+    return (stats["cell_updates"] * (40 + 8 * n) + stats["cells_inserted"] * (28 + 8 * n)
+            + stats["cells_prune_scanned"] * (45 + 8 / alpha))
+
+
+# per-phase share of the model above (bytes per cell handled by that phase)
+def phase_bytes(stats, n, alpha):
+    U, I, S = stats["cell_updates"], stats["cells_inserted"], stats["cells_prune_scanned"]
+    return {"grow": 16 * U + (28 + 8 * n) * I, "link": 0, "passA": (16 + 8 * n) * U, "passB": 8 * U,
+            "mark": 17 * S, "compact": 16 * S, "rebuild": (8 / alpha + 12) * S, "relink": 0, "sum": 0, "correct": 0}
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock + throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.stop_flag, self.sm, self.reasons, self.max_mhz = index, False, [], set(), None
+
+    def run(self):
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            h = nv.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)
+            names = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown",
+                     0x4: "sw_power_cap", 0x80: "hw_power_brake_slowdown"}
+            while not self.stop_flag:
+                self.sm.append(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksEventReasons(h) if hasattr(nv, "nvmlDeviceGetCurrentClocksEventReasons") \
+                    else nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+                for bit, nm in names.items():
+                    if r & bit:
+                        self.reasons.add(nm)
+                time.sleep(0.02)
+        except Exception as e:  # noqa: BLE001
+            self.reasons.add(f"nvml_unavailable:{type(e).__name__}")
+
+    def result(self):
+        self.stop_flag = True
+        self.join(timeout=2)
+        return {"sm_mhz": float(np.median(self.sm)) if self.sm else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.sm)}
+
+
+def drive(g, cfg):
+    """One propagation job on an initialised context (the timed call sequence)."""
+    if cfg.get("t_meas"):
+        for tm, z in zip(cfg["t_meas"], cfg["z"]):
+            g.run(tm, prune_every=cfg["prune_every"])
+            g.correct(z, cfg["R"])
+            g.prune()
+    elif cfg.get("t_end") is not None:
+        g.run(cfg["t_end"], prune_every=cfg["prune_every"])
+    else:
+        g.run(1e300, max_steps=cfg["steps"], prune_every=cfg["prune_every"])
+
+
+def drive_oracle(o, cfg, budget_s):
+    """Same call sequence on the CPU oracle, stopped after budget_s seconds. Returns (updates, seconds)."""
+    t0, upd, k = time.perf_counter(), 0, 0
+    t_end = cfg.get("t_end") if cfg.get("t_end") is not None else (cfg["t_meas"][-1] if cfg.get("t_meas") else 1e300)
+    max_steps = cfg.get("steps") or 1 << 62
+    while o.time() < t_end and k < max_steps and time.perf_counter() - t0 < budget_s:
+        o.step(t_end - o.time() if t_end < 1e299 else 0.0)
+        upd += o.count()
+        k += 1
+        if cfg["prune_every"] and k % cfg["prune_every"] == 0:
+            o.prune()
+    return upd, time.perf_counter() - t0, k
+
+
+def make_oracle(cfg):
+    from oracle.binding import Oracle
+    o = Oracle(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfg["cfl"])
+    o.init_gaussian(cfg["mean"], cfg["cov"])
+    return o
+
+
+def run_reference(args, cfg):
+    """--impl reference: the CPU oracle as it stands, each step a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    budget = 6.0
+    upd_tot, sec_tot, ksteps = 0, 0.0, 0
+    for it in range(args.warmup + args.steps):
+        o = make_oracle(cfg)
+        upd, sec, k = drive_oracle(o, cfg, budget)
+        if it >= args.warmup:
+            upd_tot, sec_tot, ksteps = upd_tot + upd, sec_tot + sec, k
+    val = upd_tot / sec_tot
+    sample = f"first {ksteps} integration steps of {cfg['name']} from its initial state (<= {budget:.0f} s of CPU per bench step)"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * sec_tot / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": {"workload": cfg["name"], "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="cfg2")
+    ap.add_argument("--impl", default="ours")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    cfg = workload(args.workload)
+    if args.impl == "reference":
+        return run_reference(args, cfg)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2508_13986_b200 import Gbees
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device: there is no CPU fallback"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    n, alpha = cfg["n"], 0.5
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        g = Gbees(n, cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfg["cfl"], max_cells=cfg["max_cells"],
+                  load_factor=alpha, device=local, stream=stream.cuda_stream)
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2
+
+        def job(profile=False):
+            g.init_gaussian(cfg["mean"], cfg["cov"])
+            flush.zero_()
+            g.profile(profile)
+            l0 = g.stats()["launches"]
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            drive(g, cfg)
+            e1.record(stream)
+            e1.synchronize()
+            st = g.stats()
+            st["launches"] -= l0
+            return e0.elapsed_time(e1), st
+
+        for _ in range(max(args.warmup, 3)):
+            job()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+        sampler = ClockSampler(local)
+        sampler.start()
+        ms_tot, upd_tot, launches, st = 0.0, 0, 0, None
+        for _ in range(args.steps):
+            ms, st = job()
+            ms_tot, upd_tot, launches = ms_tot + ms, upd_tot + st["cell_updates"], launches + st["launches"]
+        torch.cuda.synchronize()
+        clocks = sampler.result()
+        if world > 1:
+            dist.barrier()
+            t = torch.tensor([ms_tot], device="cuda"); dist.all_reduce(t, op=dist.ReduceOp.MAX); ms_max = t.item()
+            u = torch.tensor([upd_tot], device="cuda", dtype=torch.float64); dist.all_reduce(u); upd_all = u.item()
+        else:
+            ms_max, upd_all = ms_tot, upd_tot
+
+        # per-phase CUDA-event timing of one more job (same workload, same launch configuration)
+        ms_prof, st_prof = job(profile=True)
+        prof = g.profile(False)
+        pb = phase_bytes(st_prof, n, alpha)
+        phases = {k: {"ms": round(v[0], 4), "launches": v[1],
+                      "algo_GBps": (pb.get(k, 0) / (v[0] * 1e-3) / 1e9 if v[0] > 0 else None)}
+                  for k, v in prof.items() if v[1]}
+        dom = max(phases, key=lambda k: phases[k]["ms"])
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))) if os.path.exists(
+            os.path.join(ROOT, "MEASURED_PEAKS.json")) else None
+        peak, peak_src = (peaks["hbm_gbs"], "measured") if peaks else (6650.0, "fallback")
+        job_GBps = algo_bytes(st, n, alpha) / (ms_tot / args.steps * 1e-3) / 1e9
+        dom_GBps = phases[dom]["algo_GBps"] or 0.0
+        roofline = {"bound": "hbm", "kernel": dom, "achieved": dom_GBps, "peak": peak, "unit": "GB/s",
+                    "frac": dom_GBps / peak, "traffic": None, "peak_source": peak_src,
+                    "whole_job": {"achieved": job_GBps, "frac": job_GBps / peak,
+                                  "frac_of_8TBps": job_GBps / 8000.0, "algo_bytes_per_job": algo_bytes(st, n, alpha)},
+                    "phases": phases}
+
+        # e2e: host buffers in, host buffers out, every job
+        nmax = cfg["max_cells"]
+        hk = torch.empty((nmax, n), dtype=torch.int32).pin_memory() if nmax * n * 4 < (4 << 30) else None
+        import ctypes as C
+        from paper_2508_13986_b200.binding import lib
+        e2e_ms, e2e_upd, d2h = 0.0, 0, 0
+        if hk is not None:
+            hp = torch.empty(nmax, dtype=torch.float64).pin_memory()
+            for it in range(2 + args.steps):
+                flush.zero_(); torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                g.init_gaussian(np.asarray(cfg["mean"], dtype=np.float64), np.asarray(cfg["cov"], dtype=np.float64))
+                drive(g, cfg)
+                cnt = C.c_int64()
+                rc = lib().gbees_export(g._h, hk.data_ptr(), hp.data_ptr(), nmax, C.byref(cnt))
+                assert rc == 0
+                dt_ = time.perf_counter() - t0
+                if it >= 2:
+                    e2e_ms += 1e3 * dt_; e2e_upd += g.stats()["cell_updates"]; d2h = cnt.value * (4 * n + 8)
+        e2e = {"value": (e2e_upd / (e2e_ms * 1e-3) * world) if e2e_ms else None, "unit": UNIT,
+               "h2d_bytes_per_step": 8 * (n + n * n), "d2h_bytes_per_step": d2h,
+               "ms_per_step": e2e_ms / args.steps if e2e_ms else None}
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        o = make_oracle(cfg)
+        upd, sec, k = drive_oracle(o, cfg, 15.0)
+        cpu = {"value": upd / sec, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": f"first {k} integration steps of {cfg['name']} ({upd} cell-updates, {sec:.1f} s, 1 thread of {os.cpu_count()} host cores)"}
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": upd_all / (ms_max * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg["name"], "n": n, "dx": cfg["dx"][0], "threshold": cfg["thresh"],
+                       "integration_steps_per_job": st["steps"], "prunes_per_job": st["prunes"],
+                       "cell_updates_per_job": st["cell_updates"], "final_cells": st["n_cells"],
+                       "parallelism": "replicas only" if world > 1 else "1 GPU",
+                       "l2": "256 MiB memset between jobs (flush)"},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu}))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -66,7 +66,27 @@ typedef struct gbees_stats_t {
     double mass;            /* mass before the last normalisation (1 - mass left the grid) */
     int64_t cell_updates;   /* sum over steps of the active-cell count after grow */
     int64_t table_slots;    /* hashtable capacity in slots */
+    int64_t launches;       /* kernel + memset launches issued by this context so far */
+    int64_t cells_inserted;      /* cells created by grow since init */
+    int64_t cells_prune_scanned; /* sum over prunes of the cell count scanned */
+    int64_t prunes;              /* prunes since init */
 } gbees_stats_t;
+
+/* phases of the hot path, for launch accounting and optional CUDA-event timing */
+enum {
+    GBEES_PH_GROW = 0,  /* a1: grow (insert downwind targets) */
+    GBEES_PH_LINK,      /* adjacency of the new cells + their CFL terms (a2/a3) */
+    GBEES_PH_PASSA,     /* a2+a4: face velocities, upwind-owner CTU fluxes */
+    GBEES_PH_PASSB,     /* a5+a6: gather neighbour fluxes, update, mass sum, dt/t bookkeeping */
+    GBEES_PH_MARK,      /* a7: prune marking */
+    GBEES_PH_COMPACT,   /* a7: decoupled-lookback scan + stream compaction */
+    GBEES_PH_REBUILD,   /* a7/a0: hashtable clear + re-insert */
+    GBEES_PH_RELINK,    /* adjacency + CFL maximum for all cells */
+    GBEES_PH_SUM,       /* a6: mass sum + renormalise outside a step */
+    GBEES_PH_CORRECT,   /* a8 */
+    GBEES_PH_RUN,       /* a9: persistent cooperative step loop (whole launch) */
+    GBEES_PHASES
+};
 
 /* Fill *opts with the defaults (max_cells = 1<<20, load_factor 0.5, cfl 0.9, hi_res 1, MC). */
 int gbees_default_opts(gbees_opts* opts /*host*/);
@@ -112,6 +132,10 @@ int gbees_run(gbees_ctx* ctx, double t_target, int64_t max_steps, int prune_ever
 int gbees_count(gbees_ctx* ctx, int64_t* count /*host*/);
 int gbees_time(gbees_ctx* ctx, double* t /*host*/);
 int gbees_stats(gbees_ctx* ctx, gbees_stats_t* out /*host*/);
+/* Read-and-reset the per-phase accumulators (phase_ms, phase_launches: host [GBEES_PHASES],
+ * nullable), then switch CUDA-event timing of every phase on/off. Synchronises the stream.
+ * Launch counts are always kept; milliseconds only while profiling is enabled. */
+int gbees_profile(gbees_ctx* ctx, int enable, double* phase_ms, int64_t* phase_launches);
 const char* gbees_last_error(gbees_ctx* ctx);
 int gbees_clear_error(gbees_ctx* ctx);
 

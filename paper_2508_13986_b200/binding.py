@@ -26,7 +26,10 @@ class Opts(C.Structure):
 class Stats(C.Structure):
     _fields_ = [("n_cells", C.c_int64), ("n_inserted", C.c_int64), ("n_pruned", C.c_int64), ("steps", C.c_int64),
                 ("t", C.c_double), ("dt", C.c_double), ("mass", C.c_double), ("cell_updates", C.c_int64),
-                ("table_slots", C.c_int64)]
+                ("table_slots", C.c_int64), ("launches", C.c_int64),
+                ("cells_inserted", C.c_int64), ("cells_prune_scanned", C.c_int64), ("prunes", C.c_int64)]
+
+PHASES = ["grow", "link", "passA", "passB", "mark", "compact", "rebuild", "relink", "sum", "correct", "run"]
 
 
 def lib_path():
@@ -55,6 +58,7 @@ def lib():
         L.gbees_count.argtypes = [vp, C.POINTER(C.c_int64)]
         L.gbees_time.argtypes = [vp, dp]
         L.gbees_stats.argtypes = [vp, C.POINTER(Stats)]
+        L.gbees_profile.argtypes = [vp, C.c_int, dp, C.POINTER(C.c_int64)]
         L.gbees_last_error.argtypes = [vp]
         L.gbees_last_error.restype = C.c_char_p
         L.gbees_clear_error.argtypes = [vp]
@@ -150,6 +154,13 @@ class Gbees:
         s = Stats()
         self._chk(lib().gbees_stats(self._h, C.byref(s)))
         return {k: getattr(s, k) for k, _ in Stats._fields_}
+
+    def profile(self, enable):
+        """Read-and-reset per-phase {name: (ms, launches)}, then switch event timing on/off."""
+        ms = (C.c_double * len(PHASES))()
+        ln = (C.c_int64 * len(PHASES))()
+        self._chk(lib().gbees_profile(self._h, int(bool(enable)), ms, ln))
+        return {k: (ms[i], ln[i]) for i, k in enumerate(PHASES)}
 
     def last_mass(self):
         return self.stats()["mass"]

@@ -5,7 +5,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgbees.so")
-SOURCES = [os.path.join(CSRC, "gbees_api.cu")]
+SOURCES = [os.path.join(CSRC, "gbees_api.cu"), os.path.join(CSRC, "gbees_ht.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("gbees_common.cuh", "gbees_kernels.cuh")] + [
     os.path.join(os.path.dirname(HERE), "include", "gbees.h")]
 
@@ -18,7 +18,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
             os.path.getmtime(LIB) >= os.path.getmtime(d) for d in DEPS if os.path.exists(d)):
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SOURCES
+    cmd = [nvcc, "--threads", "0"] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SOURCES
     subprocess.check_call(cmd)
     return LIB
 

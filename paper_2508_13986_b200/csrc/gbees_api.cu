@@ -6,6 +6,7 @@
 #include <cstring>
 #include <string>
 #include <utility>
+#include <vector>
 
 #include "../../include/gbees.h"
 #include "gbees_kernels.cuh"
@@ -52,13 +53,36 @@ __global__ void __launch_bounds__(TPB) k_mark(const __grid_constant__ Params p, 
 __global__ void __launch_bounds__(TPB) k_compact(const __grid_constant__ Params p, const __grid_constant__ Pool pool, DevState* st) {
     phase_compact(p, pool, st);
 }
-__global__ void k_after_compact(DevState* st) {
+__global__ void k_after_compact(const __grid_constant__ Params p, DevState* st) {
+    st->prune_scanned += st->N;
+    st->prunes += 1;
+    st->N_before_grow = st->N;          // old row count, read by the adjacency remap
     st->N = st->N_after_prune;
+    st->slots = table_slots_for(p, st->N);
     st->smax_bits = 0ull;
     st->tile_counter = 0u;
 }
+__global__ void k_set_slots(const __grid_constant__ Params p, DevState* st) {
+    st->slots = table_slots_for(p, min(st->N, p.cap));
+    st->smax_bits = 0ull;
+}
+__global__ void __launch_bounds__(TPB) k_clear_table(const __grid_constant__ Pool pool, const DevState* st) {
+    phase_clear_table(pool, st);
+}
+// prune: translate the adjacency through newidx (into nbr2) and clear the resized table
+__global__ void __launch_bounds__(TPB) k_remap_clear(const __grid_constant__ Params p, const __grid_constant__ Pool pool, const DevState* st) {
+    phase_remap(p, pool, st->N_before_grow, 2 * p.n);
+    phase_clear_table(pool, st);
+}
 __global__ void __launch_bounds__(TPB) k_rebuild(const __grid_constant__ Params p, const __grid_constant__ Pool pool, DevState* st) {
     phase_rebuild(p, pool, st);
+}
+// prune tail: re-insert all keys, recompute the CFL maximum, sum the masses
+template <int NDIM, int DYN>
+__global__ void __launch_bounds__(TPB) k_rebuild_smax_sum(const __grid_constant__ Params p, const __grid_constant__ Pool pool, DevState* st) {
+    phase_rebuild(p, pool, st);
+    phase_smax<NDIM, DYN>(p, pool, st);
+    phase_sum(p, pool, st);
 }
 template <int NDIM>
 __global__ void __launch_bounds__(TPB) k_init_gaussian(const __grid_constant__ Params p, const __grid_constant__ Pool pool, DevState* st,
@@ -98,8 +122,15 @@ struct gbees_ctx {
     int no_grow = 0;
     int64_t n_inserted = 0, n_pruned = 0;
     std::string err;
-    void* allocs[16] = {nullptr};
+    void* allocs[24] = {nullptr};
     int nallocs = 0;
+    // launch accounting + optional per-phase CUDA-event timing (gbees_profile)
+    int64_t launches = 0;
+    int profile = 0;
+    std::vector<cudaEvent_t> ev_free;
+    std::vector<std::pair<int, std::pair<cudaEvent_t, cudaEvent_t>>> ev_open;
+    double phase_ms[GBEES_PHASES] = {0};
+    int64_t phase_launches[GBEES_PHASES] = {0};
 };
 
 namespace {
@@ -114,6 +145,33 @@ int fail(gbees_ctx* c, int code, const std::string& msg) {
         if (e_ != cudaSuccess)                                                                        \
             return fail(c, GBEES_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e_));       \
     } while (0)
+
+// run `body` (kernel launches) as one accounted phase; with profiling on, bracket it with events
+template <typename F>
+void phase(gbees_ctx* c, int ph, int nlaunch, F&& body) {
+    c->launches += nlaunch;
+    c->phase_launches[ph] += nlaunch;
+    if (!c->profile) { body(); return; }
+    cudaEvent_t a, b;
+    auto get = [&](cudaEvent_t* e) {
+        if (c->ev_free.empty()) cudaEventCreate(e);
+        else { *e = c->ev_free.back(); c->ev_free.pop_back(); }
+    };
+    get(&a); get(&b);
+    cudaEventRecord(a, c->stream);
+    body();
+    cudaEventRecord(b, c->stream);
+    c->ev_open.push_back({ph, {a, b}});
+}
+void drain_events(gbees_ctx* c) {   // call after a stream sync
+    for (auto& e : c->ev_open) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, e.second.first, e.second.second) == cudaSuccess) c->phase_ms[e.first] += ms;
+        c->ev_free.push_back(e.second.first);
+        c->ev_free.push_back(e.second.second);
+    }
+    c->ev_open.clear();
+}
 
 template <int V> struct IC { static constexpr int value = V; };
 
@@ -173,6 +231,7 @@ bool spd_inverse(int n, const double* A, double* inv, double* det) {
 int sync_state(gbees_ctx* c) {
     CU(cudaMemcpyAsync(c->h_st, c->d_st, sizeof(DevState), cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
+    if (c->profile) drain_events(c);
     const int e = c->h_st->err;
     if (e & E_CAPACITY) return fail(c, GBEES_ERR_CAPACITY, "cell pool capacity (opts.max_cells) exceeded");
     if (e & E_TABLE_FULL) return fail(c, GBEES_ERR_CAPACITY, "hashtable full");
@@ -183,15 +242,23 @@ int sync_state(gbees_ctx* c) {
 
 // table clear + insert all + adjacency for all + sum; finish mode as in k_finish
 int rebuild_all(gbees_ctx* c, int finish_mode) {
-    CU(cudaMemsetAsync(c->pool.table, 0xFF, c->p.slots * sizeof(ulonglong2), c->stream));
-    k_rebuild<<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
-    int rc = dispatch(c, [&](auto N_, auto D_) {
-        k_link<decltype(N_)::value, decltype(D_)::value, true><<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
-        return GBEES_OK;
+    phase(c, GBEES_PH_REBUILD, 3, [&] {
+        k_set_slots<<<1, 1, 0, c->stream>>>(c->p, c->d_st);
+        k_clear_table<<<c->grid, TPB, 0, c->stream>>>(c->pool, c->d_st);
+        k_rebuild<<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
+    });
+    int rc = GBEES_OK;
+    phase(c, GBEES_PH_RELINK, 1, [&] {
+        rc = dispatch(c, [&](auto N_, auto D_) {
+            k_link<decltype(N_)::value, decltype(D_)::value, true><<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
+            return GBEES_OK;
+        });
     });
     if (rc) return fail(c, rc, "unsupported (n, dynamics) pair");
-    k_sum<<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
-    k_finish<<<1, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st, c->grid, finish_mode);
+    phase(c, GBEES_PH_SUM, 2, [&] {
+        k_sum<<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
+        k_finish<<<1, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st, c->grid, finish_mode);
+    });
     CU(cudaGetLastError());
     return GBEES_OK;
 }
@@ -214,6 +281,9 @@ int gbees_default_opts(gbees_opts* o) {
 int gbees_destroy(gbees_ctx* c) {
     if (!c) return GBEES_OK;
     cudaSetDevice(c->device);
+    cudaStreamSynchronize(c->stream);
+    drain_events(c);
+    for (cudaEvent_t e : c->ev_free) cudaEventDestroy(e);
     for (int i = 0; i < c->nallocs; ++i) cudaFree(c->allocs[i]);
     if (c->h_st) cudaFreeHost(c->h_st);
     delete c;
@@ -249,6 +319,7 @@ int gbees_create(gbees_ctx** out, int n, const double* dx, double threshold, int
     p.thresh = threshold; p.cfl = o.cfl;
     p.cap = (uint32_t)o.max_cells;
     p.slots = (uint64_t)std::ceil((double)o.max_cells / o.load_factor);
+    p.load_factor = o.load_factor;
 
     auto bail = [&](int code, const std::string& m) { fprintf(stderr, "gbees_create: %s\n", m.c_str()); gbees_destroy(c); return code; };
     cudaError_t e = cudaSetDevice(c->device);
@@ -268,6 +339,7 @@ int gbees_create(gbees_ctx** out, int n, const double* dx, double threshold, int
     if (alloc((void**)&pl.key, cap * 8) || alloc((void**)&pl.Q, cap * 8) || alloc((void**)&pl.acc, cap * 8) ||
         alloc((void**)&pl.mask, cap * 2) || alloc((void**)&pl.nbr, cap * 4 * 2 * n) ||
         alloc((void**)&pl.phi, cap * 8 * 2 * n) || alloc((void**)&pl.table, p.slots * sizeof(ulonglong2)) ||
+        alloc((void**)&pl.nbr2, cap * 4 * 2 * n) || alloc((void**)&pl.newidx, cap * 4) ||
         alloc((void**)&pl.key2, cap * 8) || alloc((void**)&pl.Q2, cap * 8) || alloc((void**)&pl.keep, cap) ||
         alloc((void**)&pl.tile_state, (size_t)(c->ntiles_max + 1) * 8) || alloc((void**)&pl.partial, (size_t)c->grid * 8) ||
         alloc((void**)&c->d_st, sizeof(DevState)))
@@ -276,7 +348,6 @@ int gbees_create(gbees_ctx** out, int n, const double* dx, double threshold, int
     std::memset(c->h_st, 0, sizeof(DevState));
     c->h_st->scale = 1.0;
     cudaMemcpyAsync(c->d_st, c->h_st, sizeof(DevState), cudaMemcpyHostToDevice, c->stream);
-    cudaMemsetAsync(pl.table, 0xFF, p.slots * sizeof(ulonglong2), c->stream);
     if ((e = cudaStreamSynchronize(c->stream)) != cudaSuccess) return bail(GBEES_ERR_CUDA, cudaGetErrorString(e));
     *out = c;
     return GBEES_OK;
@@ -365,23 +436,37 @@ int gbees_step(gbees_ctx* c, double* dt) {
     CU(cudaSetDevice(c->device));
     if (c->h_st->N == 0) return fail(c, GBEES_ERR_DEGENERATE, "empty grid");
     const uint32_t n_before = c->h_st->N;
-    k_begin<<<1, 1, 0, c->stream>>>(c->d_st, *dt);
     int rc = dispatch(c, [&](auto N_, auto D_) {
         constexpr int NN = decltype(N_)::value, DD = decltype(D_)::value;
-        if (!c->no_grow) {
-            k_grow<NN, DD><<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
-            k_link<NN, DD, false><<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
-        }
-        k_passA<NN, DD><<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
-        k_passB<NN><<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
+        phase(c, GBEES_PH_GROW, c->no_grow ? 1 : 2, [&] {
+            k_begin<<<1, 1, 0, c->stream>>>(c->d_st, *dt);
+            if (!c->no_grow) k_grow<NN, DD><<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
+        });
+        if (!c->no_grow)
+            phase(c, GBEES_PH_LINK, 1, [&] { k_link<NN, DD, false><<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st); });
+        phase(c, GBEES_PH_PASSA, 1, [&] { k_passA<NN, DD><<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st); });
+        phase(c, GBEES_PH_PASSB, 2, [&] {
+            k_passB<NN><<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
+            k_finish<<<1, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st, c->grid, 0);
+        });
         return GBEES_OK;
     });
     if (rc) return fail(c, rc, "unsupported (n, dynamics) pair");
-    k_finish<<<1, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st, c->grid, 0);
     CU(cudaGetLastError());
     if ((rc = sync_state(c))) return rc;
     c->n_inserted = (int64_t)c->h_st->N - (int64_t)n_before;
     *dt = c->h_st->dt;
+    if ((double)c->h_st->N > c->p.load_factor * (double)c->h_st->slots && c->h_st->slots < c->p.slots) {
+        // the grid outgrew the active table: rehash into a larger one (adjacency is unaffected)
+        phase(c, GBEES_PH_REBUILD, 3, [&] {
+            k_set_slots<<<1, 1, 0, c->stream>>>(c->p, c->d_st);
+            k_clear_table<<<c->grid, TPB, 0, c->stream>>>(c->pool, c->d_st);
+            k_rebuild<<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
+        });
+        // k_set_slots also reset the running CFL maximum: restore it (autonomous f: unchanged by a rehash)
+        CU(cudaMemcpyAsync(&c->d_st->smax_bits, &c->h_st->smax_bits, 8, cudaMemcpyHostToDevice, c->stream));
+        if ((rc = sync_state(c))) return rc;
+    }
     return GBEES_OK;
 }
 
@@ -391,19 +476,33 @@ int gbees_prune(gbees_ctx* c) {
     CU(cudaSetDevice(c->device));
     const uint32_t N = c->h_st->N;
     if (N == 0) return fail(c, GBEES_ERR_DEGENERATE, "empty grid");
-    CU(cudaMemsetAsync(c->pool.keep, 0, N, c->stream));
-    CU(cudaMemsetAsync(c->pool.tile_state, 0, (size_t)(c->ntiles_max + 1) * 8, c->stream));
-    CU(cudaMemsetAsync(&c->d_st->tile_counter, 0, sizeof(unsigned), c->stream));
-    int rc = dispatch(c, [&](auto N_, auto D_) {
-        k_mark<decltype(N_)::value, decltype(D_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
-        return GBEES_OK;
+    int rc = GBEES_OK;
+    phase(c, GBEES_PH_MARK, 2, [&] {
+        cudaMemsetAsync(c->pool.keep, 0, N, c->stream);
+        rc = dispatch(c, [&](auto N_, auto D_) {
+            k_mark<decltype(N_)::value, decltype(D_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
+            return GBEES_OK;
+        });
     });
     if (rc) return fail(c, rc, "unsupported (n, dynamics) pair");
-    k_compact<<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
-    k_after_compact<<<1, 1, 0, c->stream>>>(c->d_st);
+    phase(c, GBEES_PH_COMPACT, 4, [&] {
+        cudaMemsetAsync(c->pool.tile_state, 0, (size_t)((N + SCAN_TILE - 1) / SCAN_TILE + 1) * 8, c->stream);
+        cudaMemsetAsync(&c->d_st->tile_counter, 0, sizeof(unsigned), c->stream);
+        k_compact<<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
+        k_after_compact<<<1, 1, 0, c->stream>>>(c->p, c->d_st);
+    });
+    phase(c, GBEES_PH_RELINK, 1, [&] { k_remap_clear<<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st); });
     std::swap(c->pool.key, c->pool.key2);
     std::swap(c->pool.Q, c->pool.Q2);
-    if ((rc = rebuild_all(c, 1))) return rc;
+    std::swap(c->pool.nbr, c->pool.nbr2);
+    phase(c, GBEES_PH_REBUILD, 2, [&] {
+        rc = dispatch(c, [&](auto N_, auto D_) {
+            k_rebuild_smax_sum<decltype(N_)::value, decltype(D_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
+            return GBEES_OK;
+        });
+        k_finish<<<1, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st, c->grid, 1);
+    });
+    CU(cudaGetLastError());
     if ((rc = sync_state(c))) return rc;
     c->n_pruned = (int64_t)N - (int64_t)c->h_st->N;
     if (c->h_st->N == 0) return fail(c, GBEES_ERR_DEGENERATE, "prune removed every cell");
@@ -419,12 +518,14 @@ int gbees_correct(gbees_ctx* c, const double* z, const double* R) {
     double det;
     if (!spd_inverse(c->p.n, R, g.inv, &det)) return GBEES_ERR_NOT_SPD;
     for (int j = 0; j < c->p.n; ++j) g.v[j] = z[j];
-    dispatch_n(c, [&](auto N_) {
-        k_correct<decltype(N_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st, g);
-        return GBEES_OK;
+    phase(c, GBEES_PH_CORRECT, 3, [&] {
+        dispatch_n(c, [&](auto N_) {
+            k_correct<decltype(N_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st, g);
+            return GBEES_OK;
+        });
+        k_sum<<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
+        k_finish<<<1, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st, c->grid, 1);
     });
-    k_sum<<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
-    k_finish<<<1, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st, c->grid, 1);
     CU(cudaGetLastError());
     return sync_state(c);
 }
@@ -492,7 +593,26 @@ int gbees_stats(gbees_ctx* c, gbees_stats_t* s) {
     s->dt = c->h_st->dt;
     s->mass = c->h_st->mass;
     s->cell_updates = (int64_t)c->h_st->cell_updates;
-    s->table_slots = (int64_t)c->p.slots;
+    s->table_slots = (int64_t)c->h_st->slots;
+    s->launches = c->launches;
+    s->cells_inserted = (int64_t)c->h_st->inserted_total;
+    s->cells_prune_scanned = (int64_t)c->h_st->prune_scanned;
+    s->prunes = (int64_t)c->h_st->prunes;
+    return GBEES_OK;
+}
+
+int gbees_profile(gbees_ctx* c, int enable, double* phase_ms, int64_t* phase_launches) {
+    if (!c) return GBEES_ERR_ARG;
+    cudaSetDevice(c->device);
+    cudaStreamSynchronize(c->stream);
+    drain_events(c);
+    for (int k = 0; k < GBEES_PHASES; ++k) {
+        if (phase_ms) phase_ms[k] = c->phase_ms[k];
+        if (phase_launches) phase_launches[k] = c->phase_launches[k];
+        c->phase_ms[k] = 0.0;
+        c->phase_launches[k] = 0;
+    }
+    c->profile = enable;
     return GBEES_OK;
 }
 

@@ -29,7 +29,8 @@ struct Params {
     double thresh;
     double cfl;
     uint32_t cap;        // pool capacity (cells)
-    uint64_t slots;      // hashtable slots
+    uint64_t slots;      // hashtable slots allocated (= ceil(cap / load_factor))
+    double load_factor;  // rehash to a larger active table when N / slots_in_use exceeds this
 };
 
 // Mutable scalars living in device memory (one struct, read back after each API call).
@@ -49,6 +50,10 @@ struct DevState {
     unsigned long long cell_updates;
     unsigned int tile_counter;  // dynamic tile ids for the decoupled-lookback scan
     uint32_t N_after_prune;
+    unsigned long long inserted_total;   // cells created by grow since init
+    unsigned long long prune_scanned;    // sum over prunes of the cell count scanned
+    unsigned long long prunes;
+    unsigned long long slots;            // hashtable slots in use (<= Params::slots), resized at rehash
 };
 
 struct Pool {
@@ -62,6 +67,8 @@ struct Pool {
     uint64_t* key2;      // compaction double buffers
     double* Q2;
     uint8_t* keep;       // [cap]
+    uint32_t* nbr2;      // [2n][cap] adjacency double buffer (remapped at prune)
+    uint32_t* newidx;    // [cap] old row -> new row of the last compaction (NBR_NONE = pruned)
     unsigned long long* tile_state;  // scan descriptors
     double* partial;     // block partial sums
 };
@@ -185,6 +192,14 @@ __device__ __forceinline__ double cfl_term(const Params& p, const double ul[NDIM
 }
 
 // monotonised-central limiter, division-free (A3)
+// active table size for N cells: room for the grid to grow 4x before the load factor is reached
+// (a 6-D blob can grow ~2-3x in one step), never below 2^20 slots, never above the allocation
+__host__ __device__ __forceinline__ unsigned long long table_slots_for(const Params& p, unsigned long long N) {
+    unsigned long long want = (unsigned long long)((double)N * 4.0 / p.load_factor) + 1ull;
+    if (want < (1ull << 20)) want = 1ull << 20;
+    return want < p.slots ? want : p.slots;
+}
+
 __device__ __forceinline__ double mc_limit(double a, double b) {
     if (a * b <= 0.0) return 0.0;
     const double m = fmin(0.5 * fabs(a + b), fmin(2.0 * fabs(a), 2.0 * fabs(b)));

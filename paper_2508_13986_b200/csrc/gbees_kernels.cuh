@@ -83,32 +83,94 @@ __device__ __forceinline__ void for_each_target(const Params& p, uint64_t key, c
 }
 
 // ---- a1 grow (Alg. 2 without staging: atomicCAS claims the slot) ------
+// Targets are numbered t in [0, 2n + 4 C(n,2)): t < 2n is the face target (dim t>>1, side t&1);
+// the rest are edge targets (pair (j<l), side_j, side_l).
+template <int NDIM>
+struct TargetTable {
+    static constexpr int NT = 2 * NDIM + 2 * NDIM * (NDIM - 1);
+};
+template <int NDIM>
+__device__ __forceinline__ void decode_target(int t, int& j, int& sj, int& l, int& sl) {
+    if (t < 2 * NDIM) { j = t >> 1; sj = t & 1; l = -1; sl = 0; return; }
+    int e = t - 2 * NDIM;
+    sl = e & 1; sj = (e >> 1) & 1;
+    int pair = e >> 2;           // pairs in order (0,1),(0,2),...,(0,n-1),(1,2),...
+    j = 0;
+    int row = NDIM - 1;
+    while (pair >= row) { pair -= row; --row; ++j; }
+    l = j + 1 + pair;
+}
+
+// Block-cooperative: cells that newly need growing are compacted into shared memory, then the
+// (cell, target) pairs are spread over all threads, so one front cell's ~n + C(n,2) dependent
+// hashtable claims do not serialise on a single lane.
 template <int NDIM, int DYN>
 __device__ void phase_grow(const Params& p, const Pool& pool, DevState* st) {
+    constexpr int NT = TargetTable<NDIM>::NT;
+    __shared__ uint64_t s_key[TPB];
+    __shared__ uint32_t s_flag[TPB];   // bits [0,2n): outflow (2j: lower, 2j+1: upper); [16,16+2n): at range border
+    __shared__ unsigned s_cnt;
     const uint32_t N0 = st->N_before_grow;
     const double scale = st->scale;
-    for (uint32_t i = gtid(); i < N0; i += gthreads()) {
-        const uint64_t kf = pool.key[i];
-        if (kf & KEY_GROWN) continue;                 // targets already inserted (autonomous f)
-        if (!(scale * pool.Q[i] >= p.thresh)) continue;
-        int32_t c[NDIM];
-        unpack<NDIM>(p, kf, c);
-        double ul[NDIM], uu[NDIM];
-        face_velocities<NDIM, DYN>(p, c, ul, uu);
-        for_each_target<NDIM>(p, kf, c, ul, uu, [&](uint64_t tk, bool ok) {
-            if (!ok) { atomicOr(&st->err, E_KEY_RANGE); return; }
-            const uint64_t s = ht_claim(pool.table, p.slots, tk);
-            if (s == ~0ull) return;                   // already there
-            if (s == ~0ull - 1) { atomicOr(&st->err, E_TABLE_FULL); return; }
+    const uint64_t slots = st->slots;
+    const int32_t lo = (int32_t)(-p.bias), hi = (int32_t)(p.bias - 1);
+    for (uint32_t base = blockIdx.x * blockDim.x; base < N0; base += gthreads()) {
+        if (threadIdx.x == 0) s_cnt = 0;
+        __syncthreads();
+        const uint32_t i = base + threadIdx.x;
+        if (i < N0) {
+            const uint64_t kf = pool.key[i];
+            if (!(kf & KEY_GROWN) && scale * pool.Q[i] >= p.thresh) {   // autonomous f: grow once
+                int32_t c[NDIM];
+                unpack<NDIM>(p, kf, c);
+                double ul[NDIM], uu[NDIM];
+                face_velocities<NDIM, DYN>(p, c, ul, uu);
+                uint32_t f = 0;
+#pragma unroll
+                for (int j = 0; j < NDIM; ++j) {
+                    f |= (ul[j] < 0.0 ? 1u : 0u) << (2 * j);
+                    f |= (uu[j] > 0.0 ? 1u : 0u) << (2 * j + 1);
+                    f |= (c[j] <= lo ? 1u : 0u) << (16 + 2 * j);
+                    f |= (c[j] >= hi ? 1u : 0u) << (16 + 2 * j + 1);
+                }
+                const unsigned k = atomicAdd(&s_cnt, 1u);
+                s_key[k] = kf;
+                s_flag[k] = f;
+                pool.key[i] = kf | KEY_GROWN;
+            }
+        }
+        __syncthreads();
+        const unsigned total = s_cnt * NT;
+        for (unsigned w = threadIdx.x; w < total; w += blockDim.x) {
+            const unsigned cell = w / NT;
+            const int t = (int)(w - cell * NT);
+            int j, sj, l, sl;
+            decode_target<NDIM>(t, j, sj, l, sl);
+            const uint32_t f = s_flag[cell];
+            if (!((f >> (2 * j + sj)) & 1u)) continue;
+            if (l >= 0 && !((f >> (2 * l + sl)) & 1u)) continue;
+            bool bad = (f >> (16 + 2 * j + sj)) & 1u;
+            if (l >= 0) bad = bad || ((f >> (16 + 2 * l + sl)) & 1u);
+            if (bad) { atomicOr(&st->err, E_KEY_RANGE); continue; }
+            uint64_t tk = s_key[cell];
+            const uint64_t uj = 1ull << ((NDIM - 1 - j) * p.bits);
+            tk = sj ? tk + uj : tk - uj;
+            if (l >= 0) {
+                const uint64_t ulk = 1ull << ((NDIM - 1 - l) * p.bits);
+                tk = sl ? tk + ulk : tk - ulk;
+            }
+            const uint64_t s = ht_claim(pool.table, slots, tk);
+            if (s == ~0ull) continue;                 // already there
+            if (s == ~0ull - 1) { atomicOr(&st->err, E_TABLE_FULL); continue; }
             const uint32_t idx = atomicAdd(&st->N, 1u);
-            if (idx >= p.cap) { atomicOr(&st->err, E_CAPACITY); pool.table[s].y = NBR_NONE; return; }
+            if (idx >= p.cap) { atomicOr(&st->err, E_CAPACITY); pool.table[s].y = NBR_NONE; continue; }
             pool.table[s].y = idx;
             pool.key[idx] = tk;
             pool.Q[idx] = 0.0;
 #pragma unroll
             for (int d = 0; d < 2 * NDIM; ++d) pool.nbr[(size_t)d * p.cap + idx] = NBR_NONE;
-        });
-        pool.key[i] = kf | KEY_GROWN;
+        }
+        __syncthreads();
     }
 }
 
@@ -120,38 +182,42 @@ template <int NDIM, int DYN, bool ALL>
 __device__ void phase_link(const Params& p, const Pool& pool, DevState* st) {
     const uint32_t first = ALL ? 0u : st->N_before_grow;
     const uint32_t N = min(st->N, p.cap);
+    const uint32_t cnt = N - first;
+    const uint64_t slots = st->slots;
     const int32_t lo = (int32_t)(-p.bias), hi = (int32_t)(p.bias - 1);
-    double smax = 0.0;
-    for (uint32_t i = first + gtid(); i < N; i += gthreads()) {
+    // one work item per (direction, cell), direction-major: coalesced adjacency writes and the
+    // 2n dependent lookups of a cell run on 2n different threads
+    const uint64_t items = (uint64_t)cnt * (2 * NDIM);
+    for (uint64_t w = gtid(); w < items; w += gthreads()) {
+        const int d = (int)(w / cnt);
+        const uint32_t i = first + (uint32_t)(w - (uint64_t)d * cnt);
+        const int j = d >> 1, s = d & 1, od = d ^ 1;
         const uint64_t key = pool.key[i] & ~KEY_GROWN;
-        int32_t c[NDIM];
-        unpack<NDIM>(p, key, c);
-#pragma unroll
-        for (int j = 0; j < NDIM; ++j) {
-            const uint64_t uj = 1ull << ((NDIM - 1 - j) * p.bits);
-#pragma unroll
-            for (int s = 0; s < 2; ++s) {
-                const int d = 2 * j + s, od = 2 * j + (1 - s);
-                uint32_t* mine = &pool.nbr[(size_t)d * p.cap + i];
-                uint32_t val = NBR_NONE;
-                const bool ok1 = s ? (c[j] < hi) : (c[j] > lo);
-                if (ok1) {
-                    const uint32_t nb = ht_find(pool.table, p.slots, s ? key + uj : key - uj);
-                    if (nb != NBR_NONE) {
-                        val = nb;
-                        if (!ALL) atomicMin(&pool.nbr[(size_t)od * p.cap + nb], i);
-                    } else if (s ? (c[j] < hi - 1) : (c[j] > lo + 1)) {
-                        const uint32_t nb2 = ht_find(pool.table, p.slots, s ? key + 2 * uj : key - 2 * uj);
-                        if (nb2 != NBR_NONE) {
-                            val = NBR_TAG | nb2;
-                            if (!ALL) atomicMin(&pool.nbr[(size_t)od * p.cap + nb2], NBR_TAG | i);
-                        }
-                    }
+        const uint64_t uj = 1ull << ((NDIM - 1 - j) * p.bits);
+        const int32_t cj = (int32_t)((int64_t)((key >> ((NDIM - 1 - j) * p.bits)) & ((1ull << p.bits) - 1ull)) - p.bias);
+        uint32_t val = NBR_NONE;
+        if (s ? (cj < hi) : (cj > lo)) {
+            const uint32_t nb = ht_find(pool.table, slots, s ? key + uj : key - uj);
+            if (nb != NBR_NONE) {
+                val = nb;
+                if (!ALL) atomicMin(&pool.nbr[(size_t)od * p.cap + nb], i);
+            } else if (s ? (cj < hi - 1) : (cj > lo + 1)) {
+                const uint32_t nb2 = ht_find(pool.table, slots, s ? key + 2 * uj : key - 2 * uj);
+                if (nb2 != NBR_NONE) {
+                    val = NBR_TAG | nb2;
+                    if (!ALL) atomicMin(&pool.nbr[(size_t)od * p.cap + nb2], NBR_TAG | i);
                 }
-                if (ALL) *mine = val;
-                else if (val != NBR_NONE) atomicMin(mine, val);
             }
         }
+        uint32_t* mine = &pool.nbr[(size_t)d * p.cap + i];
+        if (ALL) *mine = val;
+        else if (val != NBR_NONE) atomicMin(mine, val);
+    }
+    // CFL term of the linked cells (Eq. 8): running maximum
+    double smax = 0.0;
+    for (uint32_t i = first + gtid(); i < N; i += gthreads()) {
+        int32_t c[NDIM];
+        unpack<NDIM>(p, pool.key[i] & ~KEY_GROWN, c);
         double ul[NDIM], uu[NDIM];
         face_velocities<NDIM, DYN>(p, c, ul, uu);
         smax = fmax(smax, cfl_term<NDIM>(p, ul));
@@ -289,7 +355,7 @@ __device__ void phase_passB(const Params& p, const Pool& pool, DevState* st) {
 }
 
 // plain sum of Q (init / correct / prune); same partial[] protocol as pass B
-__device__ void phase_sum(const Params& p, const Pool& pool, DevState* st) {
+__device__ inline void phase_sum(const Params& p, const Pool& pool, DevState* st) {
     const uint32_t N = min(st->N, p.cap);
     double sum = 0.0;
     for (uint32_t i = gtid(); i < N; i += gthreads()) sum += pool.Q[i];
@@ -298,7 +364,7 @@ __device__ void phase_sum(const Params& p, const Pool& pool, DevState* st) {
 }
 
 // one block: add the partials in index order, set the scale. after_step: advance t, count.
-__device__ void finish_sum(const Params& p, const Pool& pool, DevState* st, unsigned nparts, bool after_step) {
+__device__ inline void finish_sum(const Params& p, const Pool& pool, DevState* st, unsigned nparts, bool after_step) {
     double v = 0.0;
     for (unsigned k = threadIdx.x; k < nparts; k += blockDim.x) v += pool.partial[k];
     v = block_sum(v);
@@ -317,6 +383,7 @@ __device__ void finish_sum(const Params& p, const Pool& pool, DevState* st, unsi
             st->t += dt;
             st->steps += 1;
             st->cell_updates += min(st->N, p.cap);
+            st->inserted_total += min(st->N, p.cap) - st->N_before_grow;
         }
     }
 }
@@ -331,6 +398,7 @@ template <int NDIM, int DYN>
 __device__ void phase_mark(const Params& p, const Pool& pool, DevState* st) {
     const uint32_t N = min(st->N, p.cap);
     const double scale = st->scale;
+    const uint64_t slots = st->slots;
     for (uint32_t i = gtid(); i < N; i += gthreads()) {
         const uint64_t kf = pool.key[i];
         if (!(scale * pool.Q[i] >= p.thresh)) continue;
@@ -342,7 +410,7 @@ __device__ void phase_mark(const Params& p, const Pool& pool, DevState* st) {
         face_velocities<NDIM, DYN>(p, c, ul, uu);
         for_each_target<NDIM>(p, key, c, ul, uu, [&](uint64_t tk, bool ok) {
             if (!ok) return;
-            const uint32_t nb = ht_find(pool.table, p.slots, tk);
+            const uint32_t nb = ht_find(pool.table, slots, tk);
             if (nb != NBR_NONE) pool.keep[nb] = 1;
         });
     }
@@ -355,9 +423,9 @@ constexpr int SCAN_ITEMS = 8;
 constexpr int SCAN_TILE = TPB * SCAN_ITEMS;
 
 // Generic core: flags -> stable destination index; body(i, dst) is called for kept items.
-template <typename KeepFn, typename MoveFn>
+template <typename KeepFn, typename MoveFn, typename DropFn>
 __device__ void scan_compact(uint32_t N, unsigned long long* tile_state, unsigned int* tile_counter,
-                             uint32_t* total_out, KeepFn keepf, MoveFn movef) {
+                             uint32_t* total_out, KeepFn keepf, MoveFn movef, DropFn dropf) {
     __shared__ unsigned s_tile;
     __shared__ uint32_t s_warp[TPB / 32];
     __shared__ uint32_t s_prefix;
@@ -412,12 +480,14 @@ __device__ void scan_compact(uint32_t N, unsigned long long* tile_state, unsigne
         __syncthreads();
         uint32_t dst = s_prefix + woff + (incl - local);
 #pragma unroll
-        for (int k = 0; k < SCAN_ITEMS; ++k)
+        for (int k = 0; k < SCAN_ITEMS; ++k) {
             if (f[k]) movef(base + k, dst++);
+            else if (base + k < N) dropf(base + k);
+        }
     }
 }
 
-__device__ void phase_compact(const Params& p, const Pool& pool, DevState* st) {
+__device__ inline void phase_compact(const Params& p, const Pool& pool, DevState* st) {
     const uint32_t N = min(st->N, p.cap);
     const double scale = st->scale;
     const double thresh = p.thresh;
@@ -431,15 +501,74 @@ __device__ void phase_compact(const Params& p, const Pool& pool, DevState* st) {
             // the GROWN flag survives only for cells still >= p* (their targets were all kept)
             pool.key2[d] = (scale * q >= thresh) ? kf : (kf & ~KEY_GROWN);
             pool.Q2[d] = q;
-        });
+            pool.newidx[i] = d;
+        },
+        [&](uint32_t i) { pool.newidx[i] = NBR_NONE; });
+}
+
+// Adjacency after a prune, without touching the hashtable: old rows are translated through
+// newidx. A pruned direct neighbour x is replaced by the tagged two-hop cell behind it (x's own
+// direct neighbour in the same direction) if that one survives. Work item = (direction, old row).
+__device__ inline void phase_remap(const Params& p, const Pool& pool, uint32_t N_old, int ndir) {
+    const size_t cap = p.cap;
+    const uint64_t items = (uint64_t)N_old * ndir;
+    for (uint64_t w = gtid(); w < items; w += gthreads()) {
+        const int d = (int)(w / N_old);
+        const uint32_t i = (uint32_t)(w - (uint64_t)d * N_old);
+        const uint32_t ni = pool.newidx[i];
+        if (ni == NBR_NONE) continue;
+        const uint32_t v = pool.nbr[(size_t)d * cap + i];
+        uint32_t out = NBR_NONE;
+        if (v != NBR_NONE) {
+            if (v < NBR_TAG) {
+                const uint32_t nv = pool.newidx[v];
+                if (nv != NBR_NONE) out = nv;
+                else {
+                    const uint32_t y = pool.nbr[(size_t)d * cap + v];
+                    if (y < NBR_TAG) {
+                        const uint32_t ny = pool.newidx[y];
+                        if (ny != NBR_NONE) out = NBR_TAG | ny;
+                    }
+                }
+            } else {
+                const uint32_t ny = pool.newidx[v & ~NBR_TAG];
+                if (ny != NBR_NONE) out = NBR_TAG | ny;
+            }
+        }
+        pool.nbr2[(size_t)d * cap + ni] = out;
+    }
+}
+
+// clear the active part of the table (st->slots was set for the new cell count)
+__device__ inline void phase_clear_table(const Pool& pool, const DevState* st) {
+    const uint64_t slots = st->slots;
+    const ulonglong2 e = make_ulonglong2(KEY_EMPTY, KEY_EMPTY);
+    for (uint64_t s = gtid(); s < slots; s += gthreads()) pool.table[s] = e;
+}
+
+// CFL maximum over all cells (after a prune the running maximum must be recomputed)
+template <int NDIM, int DYN>
+__device__ void phase_smax(const Params& p, const Pool& pool, DevState* st) {
+    const uint32_t N = min(st->N, p.cap);
+    double smax = 0.0;
+    for (uint32_t i = gtid(); i < N; i += gthreads()) {
+        int32_t c[NDIM];
+        unpack<NDIM>(p, pool.key[i] & ~KEY_GROWN, c);
+        double ul[NDIM], uu[NDIM];
+        face_velocities<NDIM, DYN>(p, c, ul, uu);
+        smax = fmax(smax, cfl_term<NDIM>(p, ul));
+    }
+    smax = block_max(smax);
+    if (threadIdx.x == 0 && smax > 0.0) atomicMax(&st->smax_bits, (unsigned long long)__double_as_longlong(smax));
 }
 
 // after the pointer swap: insert every pool key with its row index (table was cleared)
-__device__ void phase_rebuild(const Params& p, const Pool& pool, DevState* st) {
+__device__ inline void phase_rebuild(const Params& p, const Pool& pool, DevState* st) {
     const uint32_t N = min(st->N, p.cap);
+    const uint64_t slots = st->slots;
     for (uint32_t i = gtid(); i < N; i += gthreads()) {
         const uint64_t key = pool.key[i] & ~KEY_GROWN;
-        const uint64_t s = ht_claim(pool.table, p.slots, key);
+        const uint64_t s = ht_claim(pool.table, slots, key);
         if (s >= ~0ull - 1) { atomicOr(&st->err, s == ~0ull ? E_DEGENERATE : E_TABLE_FULL); continue; }  // duplicate key
         pool.table[s].y = i;
     }
