@@ -153,6 +153,7 @@ def main():
     ap.add_argument("--workload", default="cfg2")
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--run-mode", type=int, default=0, help="gbees_run: 0 = library default, 1 = host loop of step/prune")
     args = ap.parse_args()
     cfg = workload(args.workload)
     if args.impl == "reference":
@@ -171,7 +172,7 @@ def main():
     stream = torch.cuda.Stream()
     with torch.cuda.stream(stream):
         g = Gbees(n, cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfg["cfl"], max_cells=cfg["max_cells"],
-                  load_factor=alpha, device=local, stream=stream.cuda_stream)
+                  load_factor=alpha, device=local, stream=stream.cuda_stream, run_mode=args.run_mode)
         flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2
 
         def job(profile=False):

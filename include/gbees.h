@@ -52,6 +52,7 @@ typedef struct gbees_opts {
     int limiter;         /* 0 = monotonised central, 1 = none (phi == 1, test mode) */
     int no_grow;         /* test mode: gbees_step does not grow the grid */
     int no_normalise;    /* test mode: keep raw (un-normalised) masses after step / prune */
+    int run_mode;        /* gbees_run: 0 = persistent cooperative kernel (default), 1 = host loop of step/prune */
     int device;          /* CUDA device ordinal */
     void* stream;        /* cudaStream_t to run on (e.g. torch's current stream); NULL = default */
 } gbees_opts;
@@ -136,6 +137,11 @@ int gbees_stats(gbees_ctx* ctx, gbees_stats_t* out /*host*/);
  * nullable), then switch CUDA-event timing of every phase on/off. Synchronises the stream.
  * Launch counts are always kept; milliseconds only while profiling is enabled. */
 int gbees_profile(gbees_ctx* ctx, int enable, double* phase_ms, int64_t* phase_launches);
+/* Read-and-reset the time spent per phase INSIDE the persistent kernel of gbees_run (device
+ * %globaltimer, block 0, each phase including the grid barrier that ends it). Always collected.
+ * phase_ms: host [GBEES_PHASES]; COMPACT holds keep-clear + scan + compaction, RELINK the adjacency
+ * remap + table clear, REBUILD the re-insert + CFL maximum + mass sum. */
+int gbees_run_breakdown(gbees_ctx* ctx, double* phase_ms);
 const char* gbees_last_error(gbees_ctx* ctx);
 int gbees_clear_error(gbees_ctx* ctx);
 

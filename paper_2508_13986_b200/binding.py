@@ -20,7 +20,7 @@ class GbeesError(RuntimeError):
 class Opts(C.Structure):
     _fields_ = [("max_cells", C.c_int64), ("load_factor", C.c_double), ("cfl", C.c_double),
                 ("hi_res", C.c_int), ("limiter", C.c_int), ("no_grow", C.c_int), ("no_normalise", C.c_int),
-                ("device", C.c_int), ("stream", C.c_void_p)]
+                ("run_mode", C.c_int), ("device", C.c_int), ("stream", C.c_void_p)]
 
 
 class Stats(C.Structure):
@@ -59,6 +59,7 @@ def lib():
         L.gbees_time.argtypes = [vp, dp]
         L.gbees_stats.argtypes = [vp, C.POINTER(Stats)]
         L.gbees_profile.argtypes = [vp, C.c_int, dp, C.POINTER(C.c_int64)]
+        L.gbees_run_breakdown.argtypes = [vp, dp]
         L.gbees_last_error.argtypes = [vp]
         L.gbees_last_error.restype = C.c_char_p
         L.gbees_clear_error.argtypes = [vp]
@@ -75,7 +76,7 @@ class Gbees:
     """One GBEES context on one GPU. Methods mirror the C ABI one to one."""
 
     def __init__(self, n, dx, threshold, dynamics_id, params, max_cells=1 << 20, load_factor=0.5, cfl=0.9,
-                 hi_res=1, limiter=0, no_grow=False, no_normalise=False, device=0, stream=None):
+                 hi_res=1, limiter=0, no_grow=False, no_normalise=False, run_mode=0, device=0, stream=None):
         L = lib()
         self.n = int(n)
         o = Opts()
@@ -83,6 +84,7 @@ class Gbees:
         o.max_cells, o.load_factor, o.cfl = int(max_cells), float(load_factor), float(cfl)
         o.hi_res, o.limiter, o.no_grow, o.no_normalise = int(hi_res), int(limiter), int(no_grow), int(no_normalise)
         o.device = int(device)
+        o.run_mode = int(run_mode)
         o.stream = C.c_void_p(stream) if stream else None
         self._h = C.c_void_p()
         _, dxp = _d(dx)
@@ -161,6 +163,12 @@ class Gbees:
         ln = (C.c_int64 * len(PHASES))()
         self._chk(lib().gbees_profile(self._h, int(bool(enable)), ms, ln))
         return {k: (ms[i], ln[i]) for i, k in enumerate(PHASES)}
+
+    def run_breakdown(self):
+        """Read-and-reset {phase: ms} spent inside the persistent kernel (device timer)."""
+        ms = (C.c_double * len(PHASES))()
+        self._chk(lib().gbees_run_breakdown(self._h, ms))
+        return {k: ms[i] for i, k in enumerate(PHASES) if ms[i] > 0}
 
     def last_mass(self):
         return self.stats()["mass"]

@@ -29,7 +29,7 @@ __global__ void __launch_bounds__(TPB) k_link(const __grid_constant__ Params p, 
     phase_link<NDIM, DYN, ALL>(p, pool, st);
 }
 template <int NDIM, int DYN>
-__global__ void __launch_bounds__(TPB) k_passA(const __grid_constant__ Params p, const __grid_constant__ Pool pool, DevState* st) {
+__global__ void __launch_bounds__(PassACfg<NDIM>::BLK) k_passA(const __grid_constant__ Params p, const __grid_constant__ Pool pool, DevState* st) {
     phase_passA<NDIM, DYN>(p, pool, st);
 }
 template <int NDIM>
@@ -105,6 +105,12 @@ __global__ void __launch_bounds__(TPB) k_import(const __grid_constant__ Params p
     phase_import<NDIM>(p, pool, st, keys, vals, count);
 }
 
+template <int NDIM, int DYN>
+__global__ void __launch_bounds__(TPB) k_run(const __grid_constant__ Params p, const __grid_constant__ Pool pool, DevState* st,
+                                             const __grid_constant__ RunArgs a) {
+    phase_run<NDIM, DYN>(p, pool, st, a);
+}
+
 // ------------------------------------------------------------------------------------------------
 // context
 // ------------------------------------------------------------------------------------------------
@@ -117,9 +123,12 @@ struct gbees_ctx {
     int device = 0;
     int sms = 148;
     unsigned grid = 148 * 8;
+    unsigned grid_passA = 148 * 8;
     unsigned ntiles_max = 0;
     int sticky = 0;
     int no_grow = 0;
+    int run_mode = 0;            // 0 = persistent cooperative kernel, 1 = host loop over step/prune
+    int run_blocks_per_sm = 0;
     int64_t n_inserted = 0, n_pruned = 0;
     std::string err;
     void* allocs[24] = {nullptr};
@@ -130,6 +139,8 @@ struct gbees_ctx {
     std::vector<cudaEvent_t> ev_free;
     std::vector<std::pair<int, std::pair<cudaEvent_t, cudaEvent_t>>> ev_open;
     double phase_ms[GBEES_PHASES] = {0};
+    double run_phase_ms[GBEES_PHASES] = {0};   // breakdown inside the persistent kernel (device timer)
+    int run_ns_dirty = 0;
     int64_t phase_launches[GBEES_PHASES] = {0};
 };
 
@@ -232,6 +243,17 @@ int sync_state(gbees_ctx* c) {
     CU(cudaMemcpyAsync(c->h_st, c->d_st, sizeof(DevState), cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
     if (c->profile) drain_events(c);
+    // persistent loop: fold the device-timer phase breakdown into the accumulators
+    for (int k = 0; k < GBEES_PH_RUN; ++k)
+        if (c->h_st->phase_ns[k]) {
+            c->run_phase_ms[k] += 1e-6 * (double)c->h_st->phase_ns[k];
+            c->h_st->phase_ns[k] = 0;
+            c->run_ns_dirty = 1;
+        }
+    if (c->run_ns_dirty) {
+        cudaMemsetAsync(c->d_st->phase_ns, 0, sizeof(c->h_st->phase_ns), c->stream);
+        c->run_ns_dirty = 0;
+    }
     const int e = c->h_st->err;
     if (e & E_CAPACITY) return fail(c, GBEES_ERR_CAPACITY, "cell pool capacity (opts.max_cells) exceeded");
     if (e & E_TABLE_FULL) return fail(c, GBEES_ERR_CAPACITY, "hashtable full");
@@ -309,6 +331,7 @@ int gbees_create(gbees_ctx** out, int n, const double* dx, double threshold, int
     c->device = o.device;
     c->stream = (cudaStream_t)o.stream;
     c->no_grow = o.no_grow;
+    c->run_mode = o.run_mode;
     Params& p = c->p;
     p.n = n; p.dyn = dynamics_id;
     p.bits = 63 / n > 31 ? 31 : 63 / n;
@@ -328,6 +351,7 @@ int gbees_create(gbees_ctx** out, int n, const double* dx, double threshold, int
     if ((e = cudaGetDeviceProperties(&prop, c->device)) != cudaSuccess) return bail(GBEES_ERR_CUDA, cudaGetErrorString(e));
     c->sms = prop.multiProcessorCount;
     c->grid = (unsigned)c->sms * 8u;
+    c->grid_passA = (unsigned)c->sms * 10u;
     c->ntiles_max = (p.cap + SCAN_TILE - 1) / SCAN_TILE;
     const size_t cap = p.cap;
     auto alloc = [&](void** ptr, size_t bytes) {
@@ -444,7 +468,7 @@ int gbees_step(gbees_ctx* c, double* dt) {
         });
         if (!c->no_grow)
             phase(c, GBEES_PH_LINK, 1, [&] { k_link<NN, DD, false><<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st); });
-        phase(c, GBEES_PH_PASSA, 1, [&] { k_passA<NN, DD><<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st); });
+        phase(c, GBEES_PH_PASSA, 1, [&] { k_passA<NN, DD><<<c->grid_passA, PassACfg<NN>::BLK, 0, c->stream>>>(c->p, c->pool, c->d_st); });
         phase(c, GBEES_PH_PASSB, 2, [&] {
             k_passB<NN><<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
             k_finish<<<1, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st, c->grid, 0);
@@ -558,19 +582,58 @@ int gbees_export(gbees_ctx* c, int32_t* keys, double* pv, int64_t cap, int64_t* 
     return GBEES_OK;
 }
 
-int gbees_run(gbees_ctx* c, double t_target, int64_t max_steps, int prune_every, int64_t* steps_done) {
-    if (!c) return GBEES_ERR_ARG;
-    if (c->sticky) return c->sticky;
+// host loop over gbees_step / gbees_prune: the reference behaviour of gbees_run (opts.run_mode = 1)
+static int run_host_loop(gbees_ctx* c, double t_target, int64_t max_steps, int prune_every, int64_t* steps_done) {
     int64_t k = 0;
     int rc = GBEES_OK;
     while (k < max_steps && c->h_st->t < t_target) {
-        double dt = t_target - c->h_st->t;
+        double dt = t_target < 1e299 ? t_target - c->h_st->t : 0.0;
         if ((rc = gbees_step(c, &dt))) break;
         ++k;
         if (prune_every > 0 && k % prune_every == 0 && (rc = gbees_prune(c))) break;
     }
     if (steps_done) *steps_done = k;
     return rc;
+}
+
+int gbees_run(gbees_ctx* c, double t_target, int64_t max_steps, int prune_every, int64_t* steps_done) {
+    if (!c) return GBEES_ERR_ARG;
+    if (c->sticky) return c->sticky;
+    if (steps_done) *steps_done = 0;
+    if (c->run_mode == 1) return run_host_loop(c, t_target, max_steps, prune_every, steps_done);
+    CU(cudaSetDevice(c->device));
+    if (c->h_st->N == 0) return fail(c, GBEES_ERR_DEGENERATE, "empty grid");
+    if (max_steps <= 0 || !(c->h_st->t < t_target)) return GBEES_OK;
+    const unsigned long long steps0 = c->h_st->steps;
+    const unsigned parity0 = c->h_st->parity;
+    RunArgs a{t_target, (long long)max_steps, prune_every, c->no_grow};
+    int rc = GBEES_OK;
+    phase(c, GBEES_PH_RUN, 1, [&] {
+        rc = dispatch(c, [&](auto N_, auto D_) {
+            auto kern = k_run<decltype(N_)::value, decltype(D_)::value>;
+            if (c->run_blocks_per_sm == 0) {
+                int nb = 0;
+                if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, TPB, 0) != cudaSuccess || nb < 1) return GBEES_ERR_CUDA;
+                c->run_blocks_per_sm = nb;
+            }
+            void* args[] = {(void*)&c->p, (void*)&c->pool, (void*)&c->d_st, (void*)&a};
+            cudaError_t e = cudaLaunchCooperativeKernel((void*)kern, dim3((unsigned)(c->sms * c->run_blocks_per_sm)), dim3(TPB),
+                                                        args, 0, c->stream);
+            return e == cudaSuccess ? GBEES_OK : GBEES_ERR_CUDA;
+        });
+    });
+    if (rc == GBEES_ERR_CUDA) return fail(c, rc, std::string("cooperative launch: ") + cudaGetErrorString(cudaGetLastError()));
+    if (rc) return fail(c, rc, "unsupported (n, dynamics) pair");
+    rc = sync_state(c);
+    if ((c->h_st->parity ^ parity0) & 1u) {   // odd number of prunes inside the loop: buffers swapped
+        std::swap(c->pool.key, c->pool.key2);
+        std::swap(c->pool.Q, c->pool.Q2);
+        std::swap(c->pool.nbr, c->pool.nbr2);
+    }
+    if (steps_done) *steps_done = (int64_t)(c->h_st->steps - steps0);
+    if (rc) return rc;
+    if (c->h_st->N == 0) return fail(c, GBEES_ERR_DEGENERATE, "prune removed every cell");
+    return GBEES_OK;
 }
 
 int gbees_count(gbees_ctx* c, int64_t* count) {
@@ -598,6 +661,12 @@ int gbees_stats(gbees_ctx* c, gbees_stats_t* s) {
     s->cells_inserted = (int64_t)c->h_st->inserted_total;
     s->cells_prune_scanned = (int64_t)c->h_st->prune_scanned;
     s->prunes = (int64_t)c->h_st->prunes;
+    return GBEES_OK;
+}
+
+int gbees_run_breakdown(gbees_ctx* c, double* phase_ms) {
+    if (!c || !phase_ms) return GBEES_ERR_ARG;
+    for (int k = 0; k < GBEES_PHASES; ++k) { phase_ms[k] = c->run_phase_ms[k]; c->run_phase_ms[k] = 0.0; }
     return GBEES_OK;
 }
 

@@ -53,6 +53,9 @@ struct DevState {
     unsigned long long inserted_total;   // cells created by grow since init
     unsigned long long prune_scanned;    // sum over prunes of the cell count scanned
     unsigned long long prunes;
+    unsigned int parity;                 // toggled by every prune inside the persistent loop (buffer swap)
+    unsigned int pad_;
+    unsigned long long phase_ns[12];     // persistent loop: device-timer ns per phase (index = GBEES_PH_*)
     unsigned long long slots;            // hashtable slots in use (<= Params::slots), resized at rehash
 };
 
@@ -204,6 +207,15 @@ __device__ __forceinline__ double mc_limit(double a, double b) {
     if (a * b <= 0.0) return 0.0;
     const double m = fmin(0.5 * fabs(a + b), fmin(2.0 * fabs(a), 2.0 * fabs(b)));
     return a > 0.0 ? m : -m;
+}
+
+// same limiter, cheaper: sign test on the high words instead of a product (differs from mc_limit only
+// when a*b underflows to zero, where the result is below 1e-150 anyway)
+__device__ __forceinline__ double mc_limit_fast(double a, double b) {
+    if ((__double2hiint(a) ^ __double2hiint(b)) < 0) return 0.0;
+    const double m1 = fmin(fabs(a), fabs(b));
+    const double m = fmin(0.5 * fabs(a + b), m1 + m1);
+    return copysign(m, a);
 }
 
 }  // namespace gbees

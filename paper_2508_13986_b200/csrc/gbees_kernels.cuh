@@ -247,83 +247,148 @@ __device__ __forceinline__ double step_dt(const Params& p, const DevState* st) {
 // downwind cell computes it (needs the two-hop value through the tagged adjacency slot).
 // acc_c = P_c - sum_j tau_j (F_up - F_lo) over the faces computed here; tau_j F is stored for the
 // neighbour that shares the face; mask tells pass B which faces to fetch from neighbours.
+// Thread mapping: one WARP per (tile of 32 cells, dimension j). The NDIM warps of a tile exchange
+// T_l and their partial updates through shared memory, so a thread holds the state of one cell in
+// one dimension only (few registers, 6x the threads in flight, coalesced adjacency loads).
+template <int NDIM> struct PassACfg {
+    static constexpr int GROUPS = NDIM == 1 ? 8 : NDIM == 2 ? 4 : NDIM == 3 ? 2 : NDIM == 4 ? 2 : 1;
+    static constexpr int BLK = 32 * NDIM * GROUPS;   // 256, 256, 192, 256, 160, 192
+};
+
+struct PassALocal {
+    double q0, vm, vp, ul, uu, dm, dp, T, tau;
+    uint32_t nbm, nbp, i;
+    bool valid;
+};
+
+template <int NDIM, int DYN, int J>
+__device__ __forceinline__ void passA_stage1(const Params& p, const Pool& pool, PassALocal& L) {
+    const size_t cap = p.cap;
+    const uint64_t key = pool.key[L.i] & ~KEY_GROWN;
+    L.q0 = pool.Q[L.i];
+    L.nbm = pool.nbr[(size_t)(2 * J) * cap + L.i];
+    L.nbp = pool.nbr[(size_t)(2 * J + 1) * cap + L.i];
+    L.vm = L.nbm != NBR_NONE ? pool.Q[L.nbm & ~NBR_TAG] : 0.0;   // tagged slot: the two-hop value
+    L.vp = L.nbp != NBR_NONE ? pool.Q[L.nbp & ~NBR_TAG] : 0.0;
+    int32_t c[NDIM];
+    unpack<NDIM>(p, key, c);
+    double x[NDIM];
+#pragma unroll
+    for (int m = 0; m < NDIM; ++m) x[m] = DADD(p.mu[m], DMUL((double)c[m], p.h[m]));
+    L.ul = dyn_f<NDIM, DYN>(p, x, J, DADD(p.mu[J], DMUL((double)c[J] - 0.5, p.h[J])));
+    L.uu = dyn_f<NDIM, DYN>(p, x, J, DADD(p.mu[J], DMUL((double)c[J] + 0.5, p.h[J])));
+    L.dm = L.q0 - (L.nbm < NBR_TAG ? L.vm : 0.0);
+    L.dp = (L.nbp < NBR_TAG ? L.vp : 0.0) - L.q0;
+    double t = 0.0;
+    if (L.ul > 0.0) t = L.ul * L.dm;
+    if (L.uu < 0.0) t = fma(L.uu, L.dp, t);
+    L.T = (0.5 * L.tau) * t;
+}
+
+// faces of dimension J owned by this cell; returns the partial update (-F_up + F_lo) and mask bits
+template <int J>
+__device__ __forceinline__ double passA_stage2(const Params& p, const Pool& pool, const PassALocal& L, double S,
+                                               unsigned& mask) {
+    const size_t cap = p.cap;
+    const bool hires = p.hi_res != 0, nolim = p.limiter != 0;
+    const double G = (L.q0 - S) + L.T;     // P*_{c,(J)} = q0 - sum_{l != J} T_l
+    const double sig = (hires && !nolim) ? mc_limit_fast(L.dm, L.dp) : 0.0;
+    const double tau = L.tau;
+    double part = 0.0;
+    {   // upper face of c
+        const double u = L.uu;
+        if (u > 0.0) {
+            const double a = tau * u;
+            const double w = hires ? (nolim ? L.dp : sig) : 0.0;
+            const double F = a * fma(0.5 * (1.0 - a), w, G);
+            part -= F;
+            if (L.nbp < NBR_TAG) pool.phi[(size_t)(2 * J + 1) * cap + L.i] = F;
+        } else if (u < 0.0) {
+            if (L.nbp < NBR_TAG) {
+                mask |= 1u << (8 + J);
+            } else if (hires) {   // upwind cell c+e^J inactive: W = 0 - P_c, W_up = P_{c+2e^J} - 0
+                const double w = nolim ? -L.q0 : mc_limit(-L.q0, L.vp);
+                const double a = tau * u;
+                part -= (-0.5 * a) * (1.0 + a) * w;
+            }
+        }
+    }
+    {   // lower face of c
+        const double u = L.ul;
+        if (u < 0.0) {
+            const double a = tau * u;
+            const double w = hires ? (nolim ? L.dm : sig) : 0.0;
+            const double F = a * fma(-0.5 * (1.0 + a), w, G);
+            part += F;
+            if (L.nbm < NBR_TAG) pool.phi[(size_t)(2 * J) * cap + L.i] = F;
+        } else if (u > 0.0) {
+            if (L.nbm < NBR_TAG) {
+                mask |= 1u << J;
+            } else if (hires) {   // upwind cell c-e^J inactive: W = P_c - 0, W_up = 0 - P_{c-2e^J}
+                const double w = nolim ? L.q0 : mc_limit(L.q0, -L.vm);
+                const double a = tau * u;
+                part += (0.5 * a) * (1.0 - a) * w;
+            }
+        }
+    }
+    return part;
+}
+
 template <int NDIM, int DYN>
 __device__ void phase_passA(const Params& p, const Pool& pool, DevState* st) {
+    constexpr int GROUPS = PassACfg<NDIM>::GROUPS;
+    __shared__ double sT[GROUPS][NDIM][32];
+    __shared__ double sPart[GROUPS][NDIM][32];
+    __shared__ unsigned sMask[GROUPS][NDIM][32];
     const uint32_t N = min(st->N, p.cap);
     const double dt = step_dt(p, st);
-    double tau[NDIM];
-#pragma unroll
-    for (int j = 0; j < NDIM; ++j) tau[j] = dt / p.h[j];
-    const size_t cap = p.cap;
-    for (uint32_t i = gtid(); i < N; i += gthreads()) {
-        const uint64_t key = pool.key[i] & ~KEY_GROWN;
-        int32_t c[NDIM];
-        unpack<NDIM>(p, key, c);
-        const double q0 = pool.Q[i];
-        double qm[NDIM], qp[NDIM], qmm[NDIM], qpp[NDIM];
-        bool hasm[NDIM], hasp[NDIM];
-#pragma unroll
-        for (int j = 0; j < NDIM; ++j) {
-            const uint32_t nm = pool.nbr[(size_t)(2 * j) * cap + i];
-            const uint32_t np = pool.nbr[(size_t)(2 * j + 1) * cap + i];
-            hasm[j] = nm < NBR_TAG;
-            hasp[j] = np < NBR_TAG;
-            const double vm = nm != NBR_NONE ? pool.Q[nm & ~NBR_TAG] : 0.0;
-            const double vp = np != NBR_NONE ? pool.Q[np & ~NBR_TAG] : 0.0;
-            qm[j] = hasm[j] ? vm : 0.0;  qmm[j] = hasm[j] ? 0.0 : vm;
-            qp[j] = hasp[j] ? vp : 0.0;  qpp[j] = hasp[j] ? 0.0 : vp;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int grp = warp / NDIM, j = warp - grp * NDIM;
+    const uint32_t tiles = (N + 31) >> 5;
+    PassALocal L;
+    L.tau = dt / p.h[j];
+    for (uint32_t tb = blockIdx.x * GROUPS; tb < tiles; tb += gridDim.x * GROUPS) {   // block-uniform
+        const uint32_t tile = tb + grp;
+        L.i = tile * 32 + lane;
+        L.valid = grp < GROUPS && L.i < N;
+        L.T = 0.0;
+        if (L.valid) {
+            switch (j) {
+                case 0: passA_stage1<NDIM, DYN, 0>(p, pool, L); break;
+                case 1: if constexpr (NDIM > 1) passA_stage1<NDIM, DYN, 1>(p, pool, L); break;
+                case 2: if constexpr (NDIM > 2) passA_stage1<NDIM, DYN, 2>(p, pool, L); break;
+                case 3: if constexpr (NDIM > 3) passA_stage1<NDIM, DYN, 3>(p, pool, L); break;
+                case 4: if constexpr (NDIM > 4) passA_stage1<NDIM, DYN, 4>(p, pool, L); break;
+                case 5: if constexpr (NDIM > 5) passA_stage1<NDIM, DYN, 5>(p, pool, L); break;
+            }
         }
-        double ul[NDIM], uu[NDIM];
-        face_velocities<NDIM, DYN>(p, c, ul, uu);
-        double T[NDIM];
-#pragma unroll
-        for (int l = 0; l < NDIM; ++l)
-            T[l] = 0.5 * tau[l] * (fmax(ul[l], 0.0) * (q0 - qm[l]) + fmin(uu[l], 0.0) * (qp[l] - q0));
-        double acc = q0;
+        if (grp < GROUPS) sT[grp][j][lane] = L.T;
+        __syncthreads();
+        double part = 0.0;
         unsigned mask = 0;
+        if (L.valid) {
+            double S = 0.0;
 #pragma unroll
-        for (int j = 0; j < NDIM; ++j) {
-            double G = q0;
-#pragma unroll
-            for (int l = 0; l < NDIM; ++l)
-                if (l != j) G -= T[l];
-            const double dm = q0 - qm[j], dp = qp[j] - q0;
-            const double sig = p.hi_res ? (p.limiter ? 0.0 : mc_limit(dm, dp)) : 0.0;
-            {   // upper face of c
-                const double u = uu[j];
-                if (u > 0.0) {
-                    const double w = p.hi_res ? (p.limiter ? dp : sig) : 0.0;
-                    const double F = tau[j] * (u * G + 0.5 * u * (1.0 - tau[j] * u) * w);
-                    acc -= F;
-                    if (hasp[j]) pool.phi[(size_t)(2 * j + 1) * cap + i] = F;
-                } else if (u < 0.0) {
-                    if (hasp[j]) {
-                        mask |= 1u << (8 + j);
-                    } else if (p.hi_res) {   // upwind cell c+e^j inactive: W = 0 - P_c, W_up = P_{c+2e^j} - 0
-                        const double w = p.limiter ? -q0 : mc_limit(-q0, qpp[j]);
-                        acc -= tau[j] * (0.5 * (-u) * (1.0 + tau[j] * u) * w);
-                    }
-                }
-            }
-            {   // lower face of c
-                const double u = ul[j];
-                if (u < 0.0) {
-                    const double w = p.hi_res ? (p.limiter ? dm : sig) : 0.0;
-                    const double F = tau[j] * (u * G + 0.5 * (-u) * (1.0 + tau[j] * u) * w);
-                    acc += F;
-                    if (hasm[j]) pool.phi[(size_t)(2 * j) * cap + i] = F;
-                } else if (u > 0.0) {
-                    if (hasm[j]) {
-                        mask |= 1u << j;
-                    } else if (p.hi_res) {   // upwind cell c-e^j inactive: W = P_c - 0, W_up = 0 - P_{c-2e^j}
-                        const double w = p.limiter ? q0 : mc_limit(q0, -qmm[j]);
-                        acc += tau[j] * (0.5 * u * (1.0 - tau[j] * u) * w);
-                    }
-                }
+            for (int l = 0; l < NDIM; ++l) S += sT[grp][l][lane];
+            switch (j) {
+                case 0: part = passA_stage2<0>(p, pool, L, S, mask); break;
+                case 1: part = passA_stage2<1>(p, pool, L, S, mask); break;
+                case 2: part = passA_stage2<2>(p, pool, L, S, mask); break;
+                case 3: part = passA_stage2<3>(p, pool, L, S, mask); break;
+                case 4: part = passA_stage2<4>(p, pool, L, S, mask); break;
+                case 5: part = passA_stage2<5>(p, pool, L, S, mask); break;
             }
         }
-        pool.acc[i] = acc;
-        pool.mask[i] = (uint16_t)mask;
+        if (grp < GROUPS) { sPart[grp][j][lane] = part; sMask[grp][j][lane] = mask; }
+        __syncthreads();
+        if (L.valid && j == 0) {
+            double acc = L.q0;
+            unsigned m = 0;
+#pragma unroll
+            for (int l = 0; l < NDIM; ++l) { acc += sPart[grp][l][lane]; m |= sMask[grp][l][lane]; }
+            pool.acc[L.i] = acc;
+            pool.mask[L.i] = (uint16_t)m;
+        }
     }
 }
 
@@ -667,6 +732,141 @@ __device__ void phase_import(const Params& p, const Pool& pool, DevState* st, co
         if (!ok) { atomicOr(&st->err, E_KEY_RANGE); for (int j = 0; j < NDIM; ++j) c[j] = 0; }
         pool.key[i] = pack<NDIM>(p, c);
         pool.Q[i] = vals[i];
+    }
+}
+
+}  // namespace gbees
+
+#include <cooperative_groups.h>
+
+namespace gbees {
+
+struct RunArgs {
+    double t_target;
+    long long max_steps;
+    int prune_every;
+    int no_grow;
+};
+
+// pass B + mass sum + step bookkeeping without an extra barrier: the last block to finish (ticket)
+// adds the per-block partials in index order (deterministic) and closes the step.
+template <int NDIM>
+__device__ void phase_passB_finish(const Params& p, const Pool& pool, DevState* st) {
+    __shared__ bool s_last;
+    phase_passB<NDIM>(p, pool, st);
+    if (threadIdx.x == 0) {
+        __threadfence();
+        s_last = atomicAdd(&st->ticket, 1u) == gridDim.x - 1;
+    }
+    __syncthreads();
+    if (s_last) {
+        __threadfence();
+        finish_sum(p, pool, st, gridDim.x, true);
+        if (threadIdx.x == 0) st->ticket = 0;
+    }
+}
+
+// ---- a9 persistent cooperative step loop -----------------------------------------
+// Same phases, same order and same arithmetic as gbees_step / gbees_prune; grid.sync() replaces the
+// kernel boundaries. 4 barriers per step: grow | link | pass A | pass B + finish.
+template <int NDIM, int DYN>
+__device__ void phase_run(const Params& p, Pool pool, DevState* st, const RunArgs a) {
+    namespace cg = cooperative_groups;
+    cg::grid_group grid = cg::this_grid();
+    long long k = 0;
+    unsigned long long t_last = 0;
+    if (gtid() == 0) asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t_last));
+    // attribute the time since the previous tick (phase body + its barrier) to phase `ph`
+    auto tick = [&](int ph) {
+        if (gtid() == 0) {
+            unsigned long long now;
+            asm volatile("mov.u64 %0, %globaltimer;" : "=l"(now));
+            st->phase_ns[ph] += now - t_last;
+            t_last = now;
+        }
+    };
+    for (;;) {
+        // uniform decisions: every thread reads the same state after the barrier
+        const double t = st->t;
+        if (k >= a.max_steps || !(t < a.t_target) || st->err != 0) break;
+        if (gtid() == 0) {
+            st->N_before_grow = st->N;
+            st->dt_cap = a.t_target < 1e299 ? a.t_target - t : 0.0;
+        }
+        grid.sync();
+        if (!a.no_grow) {
+            phase_grow<NDIM, DYN>(p, pool, st);
+            grid.sync();
+            tick(0);
+            if (st->N != st->N_before_grow) {
+                phase_link<NDIM, DYN, false>(p, pool, st);
+                grid.sync();
+                tick(1);
+            }
+        }
+        phase_passA<NDIM, DYN>(p, pool, st);
+        grid.sync();
+        tick(2);
+        phase_passB_finish<NDIM>(p, pool, st);
+        grid.sync();
+        tick(3);
+        ++k;
+        if (st->err != 0) break;
+        const bool do_prune = a.prune_every > 0 && (k % a.prune_every) == 0;
+        if (!do_prune) {
+            // the grid outgrew the active table: rehash into a larger one
+            if ((double)st->N > p.load_factor * (double)st->slots && st->slots < p.slots) {
+                grid.sync();
+                if (gtid() == 0) st->slots = table_slots_for(p, min(st->N, p.cap));
+                grid.sync();
+                phase_clear_table(pool, st);
+                grid.sync();
+                phase_rebuild(p, pool, st);
+                grid.sync();
+            }
+            continue;
+        }
+        // ---- prune (D3) ----
+        {
+            const uint32_t N = min(st->N, p.cap);
+            for (uint32_t i = gtid(); i < N; i += gthreads()) pool.keep[i] = 0;
+            const uint32_t ntiles = (N + SCAN_TILE - 1) / SCAN_TILE + 1;
+            for (uint32_t i = gtid(); i < ntiles; i += gthreads()) pool.tile_state[i] = 0ull;
+            if (gtid() == 0) st->tile_counter = 0u;
+        }
+        grid.sync();
+        phase_mark<NDIM, DYN>(p, pool, st);
+        grid.sync();
+        tick(4);
+        phase_compact(p, pool, st);
+        grid.sync();
+        if (gtid() == 0) {
+            st->prune_scanned += st->N;
+            st->prunes += 1;
+            st->N_before_grow = st->N;
+            st->N = st->N_after_prune;
+            st->slots = table_slots_for(p, st->N);
+            st->smax_bits = 0ull;
+            st->tile_counter = 0u;
+            st->parity ^= 1u;
+        }
+        grid.sync();
+        tick(5);
+        phase_remap(p, pool, st->N_before_grow, 2 * NDIM);
+        phase_clear_table(pool, st);
+        grid.sync();
+        tick(7);
+        { uint64_t* tk = pool.key; pool.key = pool.key2; pool.key2 = tk; }
+        { double* tq = pool.Q; pool.Q = pool.Q2; pool.Q2 = tq; }
+        { uint32_t* tn = pool.nbr; pool.nbr = pool.nbr2; pool.nbr2 = tn; }
+        phase_rebuild(p, pool, st);
+        phase_smax<NDIM, DYN>(p, pool, st);
+        phase_sum(p, pool, st);
+        grid.sync();
+        if (blockIdx.x == 0) finish_sum(p, pool, st, gridDim.x, false);
+        grid.sync();
+        tick(6);
+        if (st->N == 0 || st->err != 0) break;
     }
 }
 

@@ -158,3 +158,46 @@ def test_errors_and_edges():
     g.step()
     k, p = g.export()
     assert len(k) == 4 and p.sum() == pytest.approx(1.0, abs=1e-15)
+
+
+def oracle_run(cfg, t_end=None, steps=None):
+    o = Oracle(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfg["cfl"])
+    o.init_gaussian(cfg["mean"], cfg["cov"])
+    k = 0
+    while (t_end is None or o.time() < t_end) and (steps is None or k < steps):
+        o.step(t_end - o.time() if t_end is not None else 0.0)
+        k += 1
+        if cfg["prune_every"] and k % cfg["prune_every"] == 0:
+            o.prune()
+    return o, k
+
+
+@pytest.mark.parametrize("run_mode", [0, 1])
+def test_run_persistent_loop_config0(run_mode):
+    """a9: gbees_run (persistent cooperative kernel / host loop) == the oracle's step/prune sequence."""
+    cfg = W.config0()
+    g = G(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfg["cfl"], max_cells=cfg["max_cells"],
+          run_mode=run_mode)
+    g.init_gaussian(cfg["mean"], cfg["cov"])
+    assert g.run(1e300, max_steps=20, prune_every=1) == 20
+    o, _ = oracle_run(cfg, steps=20)
+    assert g.time() == pytest.approx(o.time(), rel=1e-14)
+    assert compare_states(*g.export(), *o.export(), cfg["thresh"], 1e-9, what="cfg0 run") <= 1e-9
+    st = g.stats()
+    assert st["steps"] == 20 and st["prunes"] == 20
+
+
+@pytest.mark.parametrize("prune_every", [0, 2, 5])
+def test_run_persistent_loop_lorenz96_to_time(prune_every):
+    cfg = W.config2()
+    cfg.update(thresh=1e-5, max_cells=1 << 20, prune_every=prune_every)
+    g = G(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfg["cfl"], max_cells=cfg["max_cells"])
+    g.init_gaussian(cfg["mean"], cfg["cov"])
+    o, k = oracle_run(cfg, t_end=0.05)
+    assert g.run(0.05, prune_every=prune_every) == k
+    assert g.time() == o.time() == 0.05
+    compare_states(*g.export(), *o.export(), cfg["thresh"], 1e-9, what="L96 run")
+    # the context stays usable call-by-call after a persistent run (buffers swapped back correctly)
+    assert abs(g.step() - o.step()) <= 1e-14
+    g.prune(); o.prune()
+    compare_states(*g.export(), *o.export(), cfg["thresh"], 1e-9, what="L96 run + step + prune")
