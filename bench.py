@@ -153,7 +153,7 @@ def main():
     ap.add_argument("--workload", default="cfg2")
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--run-mode", type=int, default=0, help="gbees_run: 0 = library default, 1 = host loop of step/prune")
+    ap.add_argument("--run-mode", type=int, default=1, help="gbees_run: 0 = persistent cooperative kernel, 1 = host loop of step/prune launches")
     args = ap.parse_args()
     cfg = workload(args.workload)
     if args.impl == "reference":
@@ -216,6 +216,9 @@ def main():
         phases = {k: {"ms": round(v[0], 4), "launches": v[1],
                       "algo_GBps": (pb.get(k, 0) / (v[0] * 1e-3) / 1e9 if v[0] > 0 else None)}
                   for k, v in prof.items() if v[1]}
+        if args.run_mode == 0:   # one persistent kernel: its bytes are the whole job's
+            phases["run"]["algo_GBps"] = algo_bytes(st_prof, n, alpha) / (phases["run"]["ms"] * 1e-3) / 1e9
+            phases["run"]["inside_ms"] = {k: round(v, 3) for k, v in g.run_breakdown().items()}
         dom = max(phases, key=lambda k: phases[k]["ms"])
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))) if os.path.exists(
             os.path.join(ROOT, "MEASURED_PEAKS.json")) else None
@@ -265,7 +268,7 @@ def main():
             "config": {"workload": cfg["name"], "n": n, "dx": cfg["dx"][0], "threshold": cfg["thresh"],
                        "integration_steps_per_job": st["steps"], "prunes_per_job": st["prunes"],
                        "cell_updates_per_job": st["cell_updates"], "final_cells": st["n_cells"],
-                       "parallelism": "replicas only" if world > 1 else "1 GPU",
+                       "parallelism": "replicas only" if world > 1 else "1 GPU", "run_mode": args.run_mode,
                        "l2": "256 MiB memset between jobs (flush)"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu}))
     if world > 1:
