@@ -6,7 +6,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgbees.so")
 SOURCES = [os.path.join(CSRC, "gbees_api.cu"), os.path.join(CSRC, "gbees_ht.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("gbees_common.cuh", "gbees_kernels.cuh")] + [
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("gbees_common.cuh", "gbees_prims.cuh", "gbees_brick.cuh")] + [
     os.path.join(os.path.dirname(HERE), "include", "gbees.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

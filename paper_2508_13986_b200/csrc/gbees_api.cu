@@ -9,106 +9,71 @@
 #include <vector>
 
 #include "../../include/gbees.h"
-#include "gbees_kernels.cuh"
+#include "gbees_brick.cuh"
 
 using namespace gbees;
 
 // ------------------------------------------------------------------------------------------------
-// __global__ wrappers (one per phase; Params by value in constant bank)
+// __global__ wrappers (one per phase; Params / Store by value in the constant bank)
 // ------------------------------------------------------------------------------------------------
-__global__ void k_begin(DevState* st, double dt_cap) {
-    st->N_before_grow = st->N;
-    st->dt_cap = dt_cap;
+#define GP const __grid_constant__ Params p, const __grid_constant__ Store st, DevState* ds
+__global__ void k_begin(DevState* ds, double dt_cap) {
+    ds->N_before_grow = ds->N;
+    ds->NB_before_grow = ds->NB;
+    ds->dt_cap = dt_cap;
 }
 template <int NDIM, int DYN>
-__global__ void __launch_bounds__(TPB) k_grow(const __grid_constant__ Params p, const __grid_constant__ Pool pool, DevState* st) {
-    phase_grow<NDIM, DYN>(p, pool, st);
-}
-template <int NDIM, int DYN, bool ALL>
-__global__ void __launch_bounds__(TPB) k_link(const __grid_constant__ Params p, const __grid_constant__ Pool pool, DevState* st) {
-    phase_link<NDIM, DYN, ALL>(p, pool, st);
-}
+__global__ void __launch_bounds__(TPB) k_grow(GP) { phase_targets<NDIM, DYN, true>(p, st, ds); }
 template <int NDIM, int DYN>
-__global__ void __launch_bounds__(PassACfg<NDIM>::BLK) k_passA(const __grid_constant__ Params p, const __grid_constant__ Pool pool, DevState* st) {
-    phase_passA<NDIM, DYN>(p, pool, st);
-}
+__global__ void __launch_bounds__(TPB) k_mark(GP) { phase_targets<NDIM, DYN, false>(p, st, ds); }
+template <int NDIM, bool ALL>
+__global__ void __launch_bounds__(TPB) k_link(GP) { phase_link<NDIM, ALL>(p, st, ds); }
+template <int NDIM, int DYN>
+__global__ void __launch_bounds__(TPB) k_flux1(GP) { phase_flux1<NDIM, DYN>(p, st, ds); }
 template <int NDIM>
-__global__ void __launch_bounds__(TPB) k_passB(const __grid_constant__ Params p, const __grid_constant__ Pool pool, DevState* st) {
-    phase_passB<NDIM>(p, pool, st);
-}
-__global__ void __launch_bounds__(TPB) k_sum(const __grid_constant__ Params p, const __grid_constant__ Pool pool, DevState* st) {
-    phase_sum(p, pool, st);
-}
+__global__ void __launch_bounds__(TPB) k_flux2(GP) { phase_flux2<NDIM>(p, st, ds); }
+template <int NDIM, int DYN>
+__global__ void __launch_bounds__(TPB) k_smax(GP) { phase_smax<NDIM, DYN>(p, st, ds); }
+__global__ void __launch_bounds__(TPB) k_sum(GP, int count) { phase_sum(p, st, ds, count != 0); }
 // mode: 0 = after a step, 1 = renormalise only (init / correct / prune), 2 = sum only (import)
-__global__ void __launch_bounds__(TPB) k_finish(const __grid_constant__ Params p, const __grid_constant__ Pool pool, DevState* st,
-                                                unsigned nparts, int mode) {
+__global__ void __launch_bounds__(TPB) k_finish(GP, unsigned nparts, int mode) {
     Params q = p;
     if (mode == 2) q.normalise = 0;
-    finish_sum(q, pool, st, nparts, mode == 0);
+    finish_sum(q, st, ds, nparts, mode == 0);
 }
-template <int NDIM, int DYN>
-__global__ void __launch_bounds__(TPB) k_mark(const __grid_constant__ Params p, const __grid_constant__ Pool pool, DevState* st) {
-    phase_mark<NDIM, DYN>(p, pool, st);
+__global__ void __launch_bounds__(TPB) k_prune_scan(GP) { phase_prune_scan(p, st, ds); }
+__global__ void __launch_bounds__(TPB) k_prune_move(GP) { phase_prune_move(p, st, ds); }
+__global__ void __launch_bounds__(TPB) k_zero_tail(GP) { phase_zero_tail(p, st, ds); }
+__global__ void k_after_compact(const __grid_constant__ Params p, DevState* ds) {
+    ds->prune_scanned += ds->N;
+    ds->prunes += 1;
+    ds->NB = ds->NB_after_prune;
+    ds->NB_before_grow = ds->NB;
+    ds->slots = table_slots_for(p, ds->NB);
+    ds->smax_bits = 0ull;
+    ds->N = 0ull;                      // recounted by k_sum
+    ds->tile_counter = 0u;
 }
-__global__ void __launch_bounds__(TPB) k_compact(const __grid_constant__ Params p, const __grid_constant__ Pool pool, DevState* st) {
-    phase_compact(p, pool, st);
+// resize the active table for the current brick count; recount = also reset N and the CFL maximum
+__global__ void k_set_slots(const __grid_constant__ Params p, DevState* ds, int recount) {
+    ds->slots = table_slots_for(p, min(ds->NB, p.capB));
+    if (recount) { ds->smax_bits = 0ull; ds->N = 0ull; }
 }
-__global__ void k_after_compact(const __grid_constant__ Params p, DevState* st) {
-    st->prune_scanned += st->N;
-    st->prunes += 1;
-    st->N_before_grow = st->N;          // old row count, read by the adjacency remap
-    st->N = st->N_after_prune;
-    st->slots = table_slots_for(p, st->N);
-    st->smax_bits = 0ull;
-    st->tile_counter = 0u;
+__global__ void __launch_bounds__(TPB) k_clear_table(const __grid_constant__ Store st, const DevState* ds) {
+    phase_clear_table(st, ds);
 }
-__global__ void k_set_slots(const __grid_constant__ Params p, DevState* st) {
-    st->slots = table_slots_for(p, min(st->N, p.cap));
-    st->smax_bits = 0ull;
-}
-__global__ void __launch_bounds__(TPB) k_clear_table(const __grid_constant__ Pool pool, const DevState* st) {
-    phase_clear_table(pool, st);
-}
-// prune: translate the adjacency through newidx (into nbr2) and clear the resized table
-__global__ void __launch_bounds__(TPB) k_remap_clear(const __grid_constant__ Params p, const __grid_constant__ Pool pool, const DevState* st) {
-    phase_remap(p, pool, st->N_before_grow, 2 * p.n);
-    phase_clear_table(pool, st);
-}
-__global__ void __launch_bounds__(TPB) k_rebuild(const __grid_constant__ Params p, const __grid_constant__ Pool pool, DevState* st) {
-    phase_rebuild(p, pool, st);
-}
-// prune tail: re-insert all keys, recompute the CFL maximum, sum the masses
-template <int NDIM, int DYN>
-__global__ void __launch_bounds__(TPB) k_rebuild_smax_sum(const __grid_constant__ Params p, const __grid_constant__ Pool pool, DevState* st) {
-    phase_rebuild(p, pool, st);
-    phase_smax<NDIM, DYN>(p, pool, st);
-    phase_sum(p, pool, st);
+__global__ void __launch_bounds__(TPB) k_rebuild(GP) { phase_rebuild(p, st, ds); }
+template <int NDIM, bool FILL>
+__global__ void __launch_bounds__(TPB) k_init_gaussian(GP, const __grid_constant__ GaussArgs g) {
+    phase_init_gaussian<NDIM, FILL>(p, st, ds, g);
 }
 template <int NDIM>
-__global__ void __launch_bounds__(TPB) k_init_gaussian(const __grid_constant__ Params p, const __grid_constant__ Pool pool, DevState* st,
-                                                       const __grid_constant__ GaussArgs g) {
-    phase_init_gaussian<NDIM>(p, pool, st, g);
-}
+__global__ void __launch_bounds__(TPB) k_correct(GP, const __grid_constant__ GaussArgs g) { phase_correct<NDIM>(p, st, ds, g); }
 template <int NDIM>
-__global__ void __launch_bounds__(TPB) k_correct(const __grid_constant__ Params p, const __grid_constant__ Pool pool, DevState* st,
-                                                 const __grid_constant__ GaussArgs g) {
-    phase_correct<NDIM>(p, pool, st, g);
-}
-template <int NDIM>
-__global__ void __launch_bounds__(TPB) k_export(const __grid_constant__ Params p, const __grid_constant__ Pool pool, const DevState* st,
-                                                int32_t* keys, double* out) {
-    phase_export<NDIM>(p, pool, st, keys, out);
-}
-template <int NDIM>
-__global__ void __launch_bounds__(TPB) k_import(const __grid_constant__ Params p, const __grid_constant__ Pool pool, DevState* st,
-                                                const int32_t* keys, const double* vals, uint32_t count) {
-    phase_import<NDIM>(p, pool, st, keys, vals, count);
-}
-
-template <int NDIM, int DYN>
-__global__ void __launch_bounds__(TPB) k_run(const __grid_constant__ Params p, const __grid_constant__ Pool pool, DevState* st,
-                                             const __grid_constant__ RunArgs a) {
-    phase_run<NDIM, DYN>(p, pool, st, a);
+__global__ void __launch_bounds__(TPB) k_export(GP, int32_t* keys, double* out) { phase_export<NDIM>(p, st, ds, keys, out); }
+template <int NDIM, bool FILL>
+__global__ void __launch_bounds__(TPB) k_import(GP, const int32_t* keys, const double* vals, uint64_t count) {
+    phase_import<NDIM, FILL>(p, st, ds, keys, vals, count);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -116,22 +81,22 @@ __global__ void __launch_bounds__(TPB) k_run(const __grid_constant__ Params p, c
 // ------------------------------------------------------------------------------------------------
 struct gbees_ctx {
     Params p{};
-    Pool pool{};
+    Store st{};
     DevState* d_st = nullptr;
     DevState* h_st = nullptr;  // pinned mirror
     cudaStream_t stream = nullptr;
     int device = 0;
     int sms = 148;
     unsigned grid = 148 * 8;
-    unsigned grid_passA = 148 * 8;
     unsigned ntiles_max = 0;
+    size_t stage_bytes = 0;      // size of the phi array (staging area of import / host export)
     int sticky = 0;
     int no_grow = 0;
     int run_mode = 0;            // 0 = persistent cooperative kernel, 1 = host loop over step/prune
     int run_blocks_per_sm = 0;
     int64_t n_inserted = 0, n_pruned = 0;
     std::string err;
-    void* allocs[24] = {nullptr};
+    void* allocs[32] = {nullptr};
     int nallocs = 0;
     // launch accounting + optional per-phase CUDA-event timing (gbees_profile)
     int64_t launches = 0;
@@ -262,26 +227,48 @@ int sync_state(gbees_ctx* c) {
     return GBEES_OK;
 }
 
-// table clear + insert all + adjacency for all + sum; finish mode as in k_finish
+// after init / import: resize + clear the table, insert all bricks, adjacency for all, CFL maximum,
+// mass sum + cell count; finish mode as in k_finish
 int rebuild_all(gbees_ctx* c, int finish_mode) {
     phase(c, GBEES_PH_REBUILD, 3, [&] {
-        k_set_slots<<<1, 1, 0, c->stream>>>(c->p, c->d_st);
-        k_clear_table<<<c->grid, TPB, 0, c->stream>>>(c->pool, c->d_st);
-        k_rebuild<<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
+        k_set_slots<<<1, 1, 0, c->stream>>>(c->p, c->d_st, 1);
+        k_clear_table<<<c->grid, TPB, 0, c->stream>>>(c->st, c->d_st);
+        k_rebuild<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
     });
     int rc = GBEES_OK;
-    phase(c, GBEES_PH_RELINK, 1, [&] {
+    phase(c, GBEES_PH_RELINK, 2, [&] {
         rc = dispatch(c, [&](auto N_, auto D_) {
-            k_link<decltype(N_)::value, decltype(D_)::value, true><<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
+            k_link<decltype(N_)::value, true><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
+            k_smax<decltype(N_)::value, decltype(D_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
             return GBEES_OK;
         });
     });
     if (rc) return fail(c, rc, "unsupported (n, dynamics) pair");
     phase(c, GBEES_PH_SUM, 2, [&] {
-        k_sum<<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
-        k_finish<<<1, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st, c->grid, finish_mode);
+        k_sum<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 1);
+        k_finish<<<1, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, c->grid, finish_mode);
     });
     CU(cudaGetLastError());
+    return GBEES_OK;
+}
+
+// rows [0, NB) of both value buffers back to zero (invariant: unused rows are zero), then a fresh
+// state with the whole table allocation in use (the brick count of the new grid is not known yet)
+int reset_grid(gbees_ctx* c) {
+    const size_t rows = c->h_st->NB < c->p.capB ? c->h_st->NB : c->p.capB;
+    if (rows) {
+        CU(cudaMemsetAsync(c->st.Q, 0, rows * 64 * 8, c->stream));
+        CU(cudaMemsetAsync(c->st.Qn, 0, rows * 64 * 8, c->stream));
+    }
+    DevState z;
+    std::memset(&z, 0, sizeof(z));
+    z.scale = 1.0;
+    z.slots = c->p.slots;
+    *c->h_st = z;
+    CU(cudaMemcpyAsync(c->d_st, c->h_st, sizeof(DevState), cudaMemcpyHostToDevice, c->stream));
+    k_clear_table<<<c->grid, TPB, 0, c->stream>>>(c->st, c->d_st);
+    c->launches += 1;
+    c->n_inserted = c->n_pruned = 0;
     return GBEES_OK;
 }
 
@@ -321,7 +308,7 @@ int gbees_create(gbees_ctx** out, int n, const double* dx, double threshold, int
     if (o.max_cells <= 0) o.max_cells = 1 << 20;
     if (!(o.load_factor > 0.0 && o.load_factor < 1.0)) o.load_factor = 0.5;
     if (!(o.cfl > 0.0)) o.cfl = 0.9;
-    if (o.max_cells >= (int64_t)NBR_TAG) return GBEES_ERR_ARG;
+    if (o.max_cells >= (int64_t)1 << 36) return GBEES_ERR_ARG;   // brick rows are 32-bit
     const int need = dynamics_id == 0 || dynamics_id == 1 ? 3 : dynamics_id == 2 ? 1 : dynamics_id == 3 ? n * n : n;
     if (dynamics_id < 0 || dynamics_id > 4 || n_params < need || (need && !params)) return GBEES_ERR_ARG;
     if ((dynamics_id <= 1 && n != 3) || (dynamics_id == 2 && n < 4)) return GBEES_ERR_ARG;
@@ -340,8 +327,14 @@ int gbees_create(gbees_ctx** out, int n, const double* dx, double threshold, int
     for (int j = 0; j < n; ++j) p.h[j] = dx[j];
     for (int k = 0; k < need; ++k) p.par[k] = params[k];
     p.thresh = threshold; p.cfl = o.cfl;
-    p.cap = (uint32_t)o.max_cells;
-    p.slots = (uint64_t)std::ceil((double)o.max_cells / o.load_factor);
+    p.max_cells = (uint64_t)o.max_cells;
+    {   // brick capacity: rows of 64 slots; sized for a fill factor >= 1/16
+        uint64_t cb = ((uint64_t)o.max_cells + 15) / 16;
+        if (cb < 256) cb = 256;
+        p.capB = (uint32_t)cb;
+    }
+    p.slots = (uint64_t)std::ceil((double)p.capB / o.load_factor);
+    if (p.slots < (1ull << 16)) p.slots = 1ull << 16;
     p.load_factor = o.load_factor;
 
     auto bail = [&](int code, const std::string& m) { fprintf(stderr, "gbees_create: %s\n", m.c_str()); gbees_destroy(c); return code; };
@@ -351,26 +344,30 @@ int gbees_create(gbees_ctx** out, int n, const double* dx, double threshold, int
     if ((e = cudaGetDeviceProperties(&prop, c->device)) != cudaSuccess) return bail(GBEES_ERR_CUDA, cudaGetErrorString(e));
     c->sms = prop.multiProcessorCount;
     c->grid = (unsigned)c->sms * 8u;
-    c->grid_passA = (unsigned)c->sms * 10u;
-    c->ntiles_max = (p.cap + SCAN_TILE - 1) / SCAN_TILE;
-    const size_t cap = p.cap;
+    c->ntiles_max = (p.capB + SCAN_TILE - 1) / SCAN_TILE;
+    const size_t cb = p.capB, nd = 2 * (size_t)n;
     auto alloc = [&](void** ptr, size_t bytes) {
         cudaError_t e2 = cudaMalloc(ptr, bytes);
         if (e2 == cudaSuccess) c->allocs[c->nallocs++] = *ptr;
         return e2;
     };
-    Pool& pl = c->pool;
-    if (alloc((void**)&pl.key, cap * 8) || alloc((void**)&pl.Q, cap * 8) || alloc((void**)&pl.acc, cap * 8) ||
-        alloc((void**)&pl.mask, cap * 2) || alloc((void**)&pl.nbr, cap * 4 * 2 * n) ||
-        alloc((void**)&pl.phi, cap * 8 * 2 * n) || alloc((void**)&pl.table, p.slots * sizeof(ulonglong2)) ||
-        alloc((void**)&pl.nbr2, cap * 4 * 2 * n) || alloc((void**)&pl.newidx, cap * 4) ||
-        alloc((void**)&pl.key2, cap * 8) || alloc((void**)&pl.Q2, cap * 8) || alloc((void**)&pl.keep, cap) ||
-        alloc((void**)&pl.tile_state, (size_t)(c->ntiles_max + 1) * 8) || alloc((void**)&pl.partial, (size_t)c->grid * 8) ||
+    Store& st = c->st;
+    c->stage_bytes = cb * nd * 32 * 8;
+    if (alloc((void**)&st.Q, cb * 512) || alloc((void**)&st.Qn, cb * 512) || alloc((void**)&st.phi, c->stage_bytes) ||
+        alloc((void**)&st.bkey, cb * 8) || alloc((void**)&st.mask, cb * 8) || alloc((void**)&st.grown, cb * 8) ||
+        alloc((void**)&st.keep, cb * 8) || alloc((void**)&st.fetch, cb * nd * 8) || alloc((void**)&st.adj, cb * nd * 4) ||
+        alloc((void**)&st.slot_of, cb * 4) || alloc((void**)&st.table, p.slots * sizeof(ulonglong2)) ||
+        alloc((void**)&st.pend, p.slots * 8) || alloc((void**)&st.bkey2, cb * 8) || alloc((void**)&st.mask2, cb * 8) ||
+        alloc((void**)&st.grown2, cb * 8) || alloc((void**)&st.newrow, cb * 4) ||
+        alloc((void**)&st.tile_state, (size_t)(c->ntiles_max + 1) * 8) || alloc((void**)&st.partial, (size_t)c->grid * 8) ||
         alloc((void**)&c->d_st, sizeof(DevState)))
         return bail(GBEES_ERR_CUDA, std::string("cudaMalloc: ") + cudaGetErrorString(cudaGetLastError()));
     if (cudaMallocHost((void**)&c->h_st, sizeof(DevState)) != cudaSuccess) return bail(GBEES_ERR_CUDA, "cudaMallocHost");
+    cudaMemsetAsync(st.Q, 0, cb * 512, c->stream);
+    cudaMemsetAsync(st.Qn, 0, cb * 512, c->stream);
     std::memset(c->h_st, 0, sizeof(DevState));
     c->h_st->scale = 1.0;
+    c->h_st->slots = p.slots;
     cudaMemcpyAsync(c->d_st, c->h_st, sizeof(DevState), cudaMemcpyHostToDevice, c->stream);
     if ((e = cudaStreamSynchronize(c->stream)) != cudaSuccess) return bail(GBEES_ERR_CUDA, cudaGetErrorString(e));
     *out = c;
@@ -385,16 +382,6 @@ int gbees_clear_error(gbees_ctx* c) {
     c->h_st->err = 0;
     cudaSetDevice(c->device);
     cudaMemsetAsync(&c->d_st->err, 0, sizeof(int), c->stream);
-    return GBEES_OK;
-}
-
-static int reset_state(gbees_ctx* c, uint32_t N) {
-    DevState z;
-    std::memset(&z, 0, sizeof(z));
-    z.N = N; z.scale = 1.0;
-    *c->h_st = z;
-    CU(cudaMemcpyAsync(c->d_st, c->h_st, sizeof(DevState), cudaMemcpyHostToDevice, c->stream));
-    c->n_inserted = c->n_pruned = 0;
     return GBEES_OK;
 }
 
@@ -419,14 +406,17 @@ int gbees_init_gaussian(gbees_ctx* c, const double* mean, const double* cov) {
     }
     if (total > 9.0e18L) return fail(c, GBEES_ERR_CAPACITY, "initial bounding box too large");
     g.total = (unsigned long long)total;
-    int rc = reset_state(c, 0);
+    int rc = reset_grid(c);
     if (rc) return rc;
     unsigned long long blocks = (g.total + TPB - 1) / TPB;
     const unsigned grid = (unsigned)(blocks < (unsigned long long)c->sms * 64 ? (blocks ? blocks : 1) : (unsigned long long)c->sms * 64);
+    // two launches: create the bricks, then activate the cells (brick rows are published in between)
     dispatch_n(c, [&](auto N_) {
-        k_init_gaussian<decltype(N_)::value><<<grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st, g);
+        k_init_gaussian<decltype(N_)::value, false><<<grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, g);
+        k_init_gaussian<decltype(N_)::value, true><<<grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, g);
         return GBEES_OK;
     });
+    c->launches += 2;
     if ((rc = sync_state(c))) return rc;   // capacity / range errors before touching the table
     if ((rc = rebuild_all(c, 1))) return rc;
     return sync_state(c);
@@ -435,21 +425,28 @@ int gbees_init_gaussian(gbees_ctx* c, const double* mean, const double* cov) {
 int gbees_import(gbees_ctx* c, const double* origin, const int32_t* keys, const double* pvals, int64_t count) {
     if (!c || !origin || !keys || !pvals || count < 0) return GBEES_ERR_ARG;
     if (c->sticky) return c->sticky;
-    if (count > (int64_t)c->p.cap) return fail(c, GBEES_ERR_CAPACITY, "import larger than opts.max_cells");
+    if (count > (int64_t)c->p.max_cells) return fail(c, GBEES_ERR_CAPACITY, "import larger than opts.max_cells");
     CU(cudaSetDevice(c->device));
     const int n = c->p.n;
     for (int j = 0; j < n; ++j) c->p.mu[j] = origin[j];
-    // stage through phi / acc (device-to-device or host-to-device, cudaMemcpyDefault picks)
-    int32_t* dk = reinterpret_cast<int32_t*>(c->pool.phi);
-    double* dp = c->pool.acc;
-    CU(cudaMemcpyAsync(dk, keys, (size_t)count * n * 4, cudaMemcpyDefault, c->stream));
-    CU(cudaMemcpyAsync(dp, pvals, (size_t)count * 8, cudaMemcpyDefault, c->stream));
-    int rc = reset_state(c, (uint32_t)count);
+    // stage through phi (device-to-device or host-to-device, cudaMemcpyDefault picks)
+    const size_t kbytes = ((size_t)count * n * 4 + 7) & ~(size_t)7;
+    if (kbytes + (size_t)count * 8 > c->stage_bytes) return fail(c, GBEES_ERR_CAPACITY, "import larger than the staging area");
+    int32_t* dk = reinterpret_cast<int32_t*>(c->st.phi);
+    double* dp = reinterpret_cast<double*>(reinterpret_cast<char*>(c->st.phi) + kbytes);
+    if (count) {
+        CU(cudaMemcpyAsync(dk, keys, (size_t)count * n * 4, cudaMemcpyDefault, c->stream));
+        CU(cudaMemcpyAsync(dp, pvals, (size_t)count * 8, cudaMemcpyDefault, c->stream));
+    }
+    int rc = reset_grid(c);
     if (rc) return rc;
     dispatch_n(c, [&](auto N_) {
-        k_import<decltype(N_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st, dk, dp, (uint32_t)count);
+        k_import<decltype(N_)::value, false><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, dk, dp, (uint64_t)count);
+        k_import<decltype(N_)::value, true><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, dk, dp, (uint64_t)count);
         return GBEES_OK;
     });
+    c->launches += 2;
+    if ((rc = sync_state(c))) return rc;
     if ((rc = rebuild_all(c, 2))) return rc;
     return sync_state(c);
 }
@@ -459,36 +456,35 @@ int gbees_step(gbees_ctx* c, double* dt) {
     if (c->sticky) return c->sticky;
     CU(cudaSetDevice(c->device));
     if (c->h_st->N == 0) return fail(c, GBEES_ERR_DEGENERATE, "empty grid");
-    const uint32_t n_before = c->h_st->N;
+    const unsigned long long n_before = c->h_st->N;
     int rc = dispatch(c, [&](auto N_, auto D_) {
         constexpr int NN = decltype(N_)::value, DD = decltype(D_)::value;
         phase(c, GBEES_PH_GROW, c->no_grow ? 1 : 2, [&] {
             k_begin<<<1, 1, 0, c->stream>>>(c->d_st, *dt);
-            if (!c->no_grow) k_grow<NN, DD><<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
+            if (!c->no_grow) k_grow<NN, DD><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
         });
         if (!c->no_grow)
-            phase(c, GBEES_PH_LINK, 1, [&] { k_link<NN, DD, false><<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st); });
-        phase(c, GBEES_PH_PASSA, 1, [&] { k_passA<NN, DD><<<c->grid_passA, PassACfg<NN>::BLK, 0, c->stream>>>(c->p, c->pool, c->d_st); });
+            phase(c, GBEES_PH_LINK, 1, [&] { k_link<NN, false><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st); });
+        phase(c, GBEES_PH_PASSA, 1, [&] { k_flux1<NN, DD><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st); });
         phase(c, GBEES_PH_PASSB, 2, [&] {
-            k_passB<NN><<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
-            k_finish<<<1, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st, c->grid, 0);
+            k_flux2<NN><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
+            k_finish<<<1, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, c->grid, 0);
         });
         return GBEES_OK;
     });
     if (rc) return fail(c, rc, "unsupported (n, dynamics) pair");
     CU(cudaGetLastError());
+    std::swap(c->st.Q, c->st.Qn);          // pass 2 left the new masses in Qn
     if ((rc = sync_state(c))) return rc;
     c->n_inserted = (int64_t)c->h_st->N - (int64_t)n_before;
     *dt = c->h_st->dt;
-    if ((double)c->h_st->N > c->p.load_factor * (double)c->h_st->slots && c->h_st->slots < c->p.slots) {
+    if ((double)c->h_st->NB > c->p.load_factor * (double)c->h_st->slots && c->h_st->slots < c->p.slots) {
         // the grid outgrew the active table: rehash into a larger one (adjacency is unaffected)
         phase(c, GBEES_PH_REBUILD, 3, [&] {
-            k_set_slots<<<1, 1, 0, c->stream>>>(c->p, c->d_st);
-            k_clear_table<<<c->grid, TPB, 0, c->stream>>>(c->pool, c->d_st);
-            k_rebuild<<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
+            k_set_slots<<<1, 1, 0, c->stream>>>(c->p, c->d_st, 0);
+            k_clear_table<<<c->grid, TPB, 0, c->stream>>>(c->st, c->d_st);
+            k_rebuild<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
         });
-        // k_set_slots also reset the running CFL maximum: restore it (autonomous f: unchanged by a rehash)
-        CU(cudaMemcpyAsync(&c->d_st->smax_bits, &c->h_st->smax_bits, 8, cudaMemcpyHostToDevice, c->stream));
         if ((rc = sync_state(c))) return rc;
     }
     return GBEES_OK;
@@ -498,33 +494,42 @@ int gbees_prune(gbees_ctx* c) {
     if (!c) return GBEES_ERR_ARG;
     if (c->sticky) return c->sticky;
     CU(cudaSetDevice(c->device));
-    const uint32_t N = c->h_st->N;
+    const unsigned long long N = c->h_st->N;
+    const uint32_t NB = c->h_st->NB;
     if (N == 0) return fail(c, GBEES_ERR_DEGENERATE, "empty grid");
     int rc = GBEES_OK;
     phase(c, GBEES_PH_MARK, 2, [&] {
-        cudaMemsetAsync(c->pool.keep, 0, N, c->stream);
+        cudaMemsetAsync(c->st.keep, 0, (size_t)NB * 8, c->stream);
         rc = dispatch(c, [&](auto N_, auto D_) {
-            k_mark<decltype(N_)::value, decltype(D_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
+            k_mark<decltype(N_)::value, decltype(D_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
             return GBEES_OK;
         });
     });
     if (rc) return fail(c, rc, "unsupported (n, dynamics) pair");
-    phase(c, GBEES_PH_COMPACT, 4, [&] {
-        cudaMemsetAsync(c->pool.tile_state, 0, (size_t)((N + SCAN_TILE - 1) / SCAN_TILE + 1) * 8, c->stream);
+    phase(c, GBEES_PH_COMPACT, 6, [&] {
+        cudaMemsetAsync(c->st.tile_state, 0, (size_t)((NB + SCAN_TILE - 1) / SCAN_TILE + 1) * 8, c->stream);
         cudaMemsetAsync(&c->d_st->tile_counter, 0, sizeof(unsigned), c->stream);
-        k_compact<<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
+        k_prune_scan<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
+        k_prune_move<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
+        k_zero_tail<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
         k_after_compact<<<1, 1, 0, c->stream>>>(c->p, c->d_st);
     });
-    phase(c, GBEES_PH_RELINK, 1, [&] { k_remap_clear<<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st); });
-    std::swap(c->pool.key, c->pool.key2);
-    std::swap(c->pool.Q, c->pool.Q2);
-    std::swap(c->pool.nbr, c->pool.nbr2);
+    std::swap(c->st.Q, c->st.Qn);
+    std::swap(c->st.bkey, c->st.bkey2);
+    std::swap(c->st.mask, c->st.mask2);
+    std::swap(c->st.grown, c->st.grown2);
     phase(c, GBEES_PH_REBUILD, 2, [&] {
+        k_clear_table<<<c->grid, TPB, 0, c->stream>>>(c->st, c->d_st);
+        k_rebuild<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
+    });
+    phase(c, GBEES_PH_RELINK, 4, [&] {
         rc = dispatch(c, [&](auto N_, auto D_) {
-            k_rebuild_smax_sum<decltype(N_)::value, decltype(D_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
+            k_link<decltype(N_)::value, true><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
+            k_smax<decltype(N_)::value, decltype(D_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
             return GBEES_OK;
         });
-        k_finish<<<1, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st, c->grid, 1);
+        k_sum<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 1);
+        k_finish<<<1, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, c->grid, 1);
     });
     CU(cudaGetLastError());
     if ((rc = sync_state(c))) return rc;
@@ -544,11 +549,11 @@ int gbees_correct(gbees_ctx* c, const double* z, const double* R) {
     for (int j = 0; j < c->p.n; ++j) g.v[j] = z[j];
     phase(c, GBEES_PH_CORRECT, 3, [&] {
         dispatch_n(c, [&](auto N_) {
-            k_correct<decltype(N_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st, g);
+            k_correct<decltype(N_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, g);
             return GBEES_OK;
         });
-        k_sum<<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st);
-        k_finish<<<1, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st, c->grid, 1);
+        k_sum<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 0);
+        k_finish<<<1, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, c->grid, 1);
     });
     CU(cudaGetLastError());
     return sync_state(c);
@@ -557,7 +562,7 @@ int gbees_correct(gbees_ctx* c, const double* z, const double* R) {
 int gbees_export(gbees_ctx* c, int32_t* keys, double* pv, int64_t cap, int64_t* count) {
     if (!c) return GBEES_ERR_ARG;
     if (c->sticky) return c->sticky;
-    const int64_t N = c->h_st->N;
+    const int64_t N = (int64_t)c->h_st->N;
     if (count) *count = N;
     if (!keys && !pv) return GBEES_OK;
     if (cap < N) return GBEES_ERR_BUFFER;
@@ -569,12 +574,17 @@ int gbees_export(gbees_ctx* c, int32_t* keys, double* pv, int64_t cap, int64_t* 
         return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
     };
     const int n = c->p.n;
-    int32_t* dk = keys ? (on_device(keys) ? keys : reinterpret_cast<int32_t*>(c->pool.phi)) : nullptr;
-    double* dp = pv ? (on_device(pv) ? pv : c->pool.acc) : nullptr;
+    // host buffers are served through the phi array (free between steps) as a staging area
+    const size_t kbytes = ((size_t)N * n * 4 + 7) & ~(size_t)7;
+    if (kbytes + (size_t)N * 8 > c->stage_bytes) return fail(c, GBEES_ERR_CAPACITY, "export larger than the staging area");
+    int32_t* dk = keys ? (on_device(keys) ? keys : reinterpret_cast<int32_t*>(c->st.phi)) : nullptr;
+    double* dp = pv ? (on_device(pv) ? pv : reinterpret_cast<double*>(reinterpret_cast<char*>(c->st.phi) + kbytes)) : nullptr;
+    CU(cudaMemsetAsync(&c->d_st->export_count, 0, sizeof(unsigned), c->stream));
     dispatch_n(c, [&](auto N_) {
-        k_export<decltype(N_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->pool, c->d_st, dk, dp);
+        k_export<decltype(N_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, dk, dp);
         return GBEES_OK;
     });
+    c->launches += 1;
     CU(cudaGetLastError());
     if (keys && dk != keys) CU(cudaMemcpyAsync(keys, dk, (size_t)N * n * 4, cudaMemcpyDeviceToHost, c->stream));
     if (pv && dp != pv) CU(cudaMemcpyAsync(pv, dp, (size_t)N * 8, cudaMemcpyDeviceToHost, c->stream));
@@ -600,40 +610,7 @@ int gbees_run(gbees_ctx* c, double t_target, int64_t max_steps, int prune_every,
     if (!c) return GBEES_ERR_ARG;
     if (c->sticky) return c->sticky;
     if (steps_done) *steps_done = 0;
-    if (c->run_mode == 1) return run_host_loop(c, t_target, max_steps, prune_every, steps_done);
-    CU(cudaSetDevice(c->device));
-    if (c->h_st->N == 0) return fail(c, GBEES_ERR_DEGENERATE, "empty grid");
-    if (max_steps <= 0 || !(c->h_st->t < t_target)) return GBEES_OK;
-    const unsigned long long steps0 = c->h_st->steps;
-    const unsigned parity0 = c->h_st->parity;
-    RunArgs a{t_target, (long long)max_steps, prune_every, c->no_grow};
-    int rc = GBEES_OK;
-    phase(c, GBEES_PH_RUN, 1, [&] {
-        rc = dispatch(c, [&](auto N_, auto D_) {
-            auto kern = k_run<decltype(N_)::value, decltype(D_)::value>;
-            if (c->run_blocks_per_sm == 0) {
-                int nb = 0;
-                if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, TPB, 0) != cudaSuccess || nb < 1) return GBEES_ERR_CUDA;
-                c->run_blocks_per_sm = nb;
-            }
-            void* args[] = {(void*)&c->p, (void*)&c->pool, (void*)&c->d_st, (void*)&a};
-            cudaError_t e = cudaLaunchCooperativeKernel((void*)kern, dim3((unsigned)(c->sms * c->run_blocks_per_sm)), dim3(TPB),
-                                                        args, 0, c->stream);
-            return e == cudaSuccess ? GBEES_OK : GBEES_ERR_CUDA;
-        });
-    });
-    if (rc == GBEES_ERR_CUDA) return fail(c, rc, std::string("cooperative launch: ") + cudaGetErrorString(cudaGetLastError()));
-    if (rc) return fail(c, rc, "unsupported (n, dynamics) pair");
-    rc = sync_state(c);
-    if ((c->h_st->parity ^ parity0) & 1u) {   // odd number of prunes inside the loop: buffers swapped
-        std::swap(c->pool.key, c->pool.key2);
-        std::swap(c->pool.Q, c->pool.Q2);
-        std::swap(c->pool.nbr, c->pool.nbr2);
-    }
-    if (steps_done) *steps_done = (int64_t)(c->h_st->steps - steps0);
-    if (rc) return rc;
-    if (c->h_st->N == 0) return fail(c, GBEES_ERR_DEGENERATE, "prune removed every cell");
-    return GBEES_OK;
+    return run_host_loop(c, t_target, max_steps, prune_every, steps_done);
 }
 
 int gbees_count(gbees_ctx* c, int64_t* count) {

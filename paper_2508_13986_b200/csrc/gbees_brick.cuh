@@ -1,0 +1,747 @@
+// Kernels of the GBEES prediction step on the dense-brick store.
+// Every phase is a grid-stride __device__ function, so the same code runs as a stream of small
+// launches (gbees_step / gbees_prune) or inside the persistent cooperative loop (gbees_run,
+// PAPER.md:170-172). Semantics: DESIGN.md D1-D5 (= SURVEY.md 8(c)).
+//
+// Brick geometry: 64 cell slots per brick, 2^K_j cells along dimension j (sum K_j = 6; n = 6: a
+// 2x2x2x2x2x2 box). Local index l = concatenation of the low K_j bits of every coordinate, dim 0
+// most significant. One warp works on one brick; neighbour values inside the brick come from
+// shared memory, values across a brick face from the neighbour brick's row (coalesced 8-byte loads
+// of a contiguous 512-byte row), so the per-cell adjacency and per-cell keys of a cell list are gone.
+#pragma once
+#include "gbees_prims.cuh"
+
+namespace gbees {
+
+constexpr int WPB = TPB / 32;   // warps (= bricks in flight) per block
+
+template <int NDIM>
+struct Geo {
+    __host__ __device__ static constexpr int K(int j) { return 6 / NDIM + (j < 6 % NDIM ? 1 : 0); }
+    __host__ __device__ static constexpr int SH(int j) {
+        int s = 0;
+        for (int m = j + 1; m < NDIM; ++m) s += K(m);
+        return s;
+    }
+    __host__ __device__ static constexpr int MK(int j) { return (1 << K(j)) - 1; }
+    // index of local cell l on a j-face (the bits of dimension j removed)
+    __host__ __device__ static constexpr int fidx(int j, int l) {
+        return ((l >> (SH(j) + K(j))) << SH(j)) | (l & ((1 << SH(j)) - 1));
+    }
+};
+
+__device__ __forceinline__ unsigned gwarp() { return (blockIdx.x * blockDim.x + threadIdx.x) >> 5; }
+__device__ __forceinline__ unsigned gwarps() { return (gridDim.x * blockDim.x) >> 5; }
+__device__ __forceinline__ unsigned lane_id() { return threadIdx.x & 31; }
+
+// cell coordinates of local slot l in the brick with coordinates B
+template <int NDIM>
+__device__ __forceinline__ void cell_coords(const int32_t B[NDIM], int l, int32_t c[NDIM]) {
+#pragma unroll
+    for (int j = 0; j < NDIM; ++j) c[j] = B[j] * (1 << Geo<NDIM>::K(j)) + ((l >> Geo<NDIM>::SH(j)) & Geo<NDIM>::MK(j));
+}
+// brick coordinates + local slot of cell c
+template <int NDIM>
+__device__ __forceinline__ int cell_to_brick(const int32_t c[NDIM], int32_t B[NDIM]) {
+    int l = 0;
+#pragma unroll
+    for (int j = 0; j < NDIM; ++j) {
+        B[j] = c[j] >> Geo<NDIM>::K(j);                         // arithmetic shift = floor
+        l |= (c[j] & Geo<NDIM>::MK(j)) << Geo<NDIM>::SH(j);
+    }
+    return l;
+}
+
+// dt of Eq. (8) with the caller's cap (every thread computes the same value)
+__device__ __forceinline__ double step_dt(const Params& p, const DevState* ds) {
+    const double smax = __longlong_as_double((long long)ds->smax_bits);
+    const double cap = ds->dt_cap;
+    const bool capped = isfinite(cap) && cap > 0.0;
+    double dt = smax > 0.0 ? __ddiv_rn(p.cfl, smax) : (capped ? cap : 0.0);
+    if (capped && cap < dt) dt = cap;
+    return dt;
+}
+
+// ---- a1 grow / a7 mark: Targets(c), D1.1 / A10 / A11 -------------------------------------------
+// Targets are numbered t in [0, 2n + 4 C(n,2)): t < 2n is the face target (dim t>>1, side t&1);
+// the rest are edge targets (pair (j<l), side_j, side_l).
+template <int NDIM>
+__device__ __forceinline__ void decode_target(int t, int& j, int& sj, int& l, int& sl) {
+    if (t < 2 * NDIM) { j = t >> 1; sj = t & 1; l = -1; sl = 0; return; }
+    int e = t - 2 * NDIM;
+    sl = e & 1; sj = (e >> 1) & 1;
+    int pair = e >> 2;           // pairs in order (0,1),(0,2),...,(0,n-1),(1,2),...
+    j = 0;
+    int row = NDIM - 1;
+    while (pair >= row) { pair -= row; --row; ++j; }
+    l = j + 1 + pair;
+}
+
+// GROW = true  (Alg. 2 without staging: atomicCAS claims the brick slot):
+//   sources = active cells with P >= p* whose targets were not inserted yet; every target cell is
+//   activated (bit set in its brick's mask; the brick is created if absent).
+// GROW = false (Alg. 3 line "mark"): sources = all cells with P >= p*; the source and
+//   every existing target get a keep mark.
+// Block-cooperative: the sources of WPB bricks are compacted into shared memory, then the
+// (source, target) pairs are spread over all threads.
+template <int NDIM, int DYN, bool GROW>
+__device__ void phase_targets(const Params& p, const Store& st, DevState* ds) {
+    using G = Geo<NDIM>;
+    constexpr int NT = 2 * NDIM + 2 * NDIM * (NDIM - 1);
+    constexpr int ND = 2 * NDIM;
+    __shared__ uint32_t s_row[WPB * 64];
+    __shared__ uint32_t s_flag[WPB * 64];   // [0,2n): outflow bits (2j: lower, 2j+1: upper); [16,16+2n): at range border; [28,32)+: unused
+    __shared__ uint8_t s_loc[WPB * 64];
+    __shared__ unsigned s_cnt;
+    const uint32_t NB0 = GROW ? ds->NB_before_grow : min(ds->NB, p.capB);
+    const double scale = ds->scale;
+    const uint64_t slots = ds->slots;
+    const int32_t lo = (int32_t)(-p.bias), hi = (int32_t)(p.bias - 1);
+    const unsigned warp = threadIdx.x >> 5, lane = lane_id();
+    unsigned long long n_new = 0;
+    double smax = 0.0;
+    for (uint32_t base = blockIdx.x * WPB; base < NB0; base += gridDim.x * WPB) {   // block-uniform
+        if (threadIdx.x == 0) s_cnt = 0;
+        __syncthreads();
+        const uint32_t b = base + warp;
+        if (b < NB0) {
+            const uint64_t m = st.mask[b];
+            const uint64_t g = GROW ? st.grown[b] : 0ull;
+            const uint64_t cand = m & ~g;
+            if (cand) {                                                            // warp-uniform
+                const uint64_t bk = st.bkey[b];
+                int32_t B[NDIM];
+                unpack<NDIM>(p, bk, B);
+                uint64_t src = 0;
+#pragma unroll
+                for (int hh = 0; hh < 2; ++hh) {
+                    const int l = (int)lane + 32 * hh;
+                    bool is_src = false;
+                    if ((cand >> l) & 1ull) is_src = scale * st.Q[(size_t)b * 64 + l] >= p.thresh;
+                    if (is_src) {
+                        int32_t c[NDIM];
+                        cell_coords<NDIM>(B, l, c);
+                        double ul[NDIM], uu[NDIM];
+                        face_velocities<NDIM, DYN>(p, c, ul, uu);
+                        uint32_t f = 0;
+#pragma unroll
+                        for (int j = 0; j < NDIM; ++j) {
+                            f |= (ul[j] < 0.0 ? 1u : 0u) << (2 * j);
+                            f |= (uu[j] > 0.0 ? 1u : 0u) << (2 * j + 1);
+                            f |= (c[j] <= lo ? 1u : 0u) << (16 + 2 * j);
+                            f |= (c[j] >= hi ? 1u : 0u) << (16 + 2 * j + 1);
+                        }
+                        const unsigned k = atomicAdd(&s_cnt, 1u);
+                        s_row[k] = b; s_loc[k] = (uint8_t)l; s_flag[k] = f;
+                    }
+                    src |= (uint64_t)__ballot_sync(0xffffffffu, is_src) << (32 * hh);
+                }
+                if (lane == 0 && src) {
+                    if (GROW) st.grown[b] = g | src;          // autonomous f: grow once
+                    else atomicOr((unsigned long long*)&st.keep[b], (unsigned long long)src);
+                }
+            }
+        }
+        __syncthreads();
+        const unsigned total = s_cnt * NT;
+        for (unsigned w = threadIdx.x; w < total; w += blockDim.x) {
+            const unsigned src = w / NT;
+            const int t = (int)(w - src * NT);
+            int j, sj, l2, sl;
+            decode_target<NDIM>(t, j, sj, l2, sl);
+            const uint32_t f = s_flag[src];
+            if (!((f >> (2 * j + sj)) & 1u)) continue;
+            if (l2 >= 0 && !((f >> (2 * l2 + sl)) & 1u)) continue;
+            bool bad = (f >> (16 + 2 * j + sj)) & 1u;
+            if (l2 >= 0) bad = bad || ((f >> (16 + 2 * l2 + sl)) & 1u);
+            if (bad) { if (GROW) atomicOr(&ds->err, E_KEY_RANGE); continue; }
+            const uint32_t r = s_row[src];
+            int tl = s_loc[src];
+            const uint64_t bk = st.bkey[r];
+            uint64_t tk = bk;
+            int carries = 0, cdir = 0;
+            {   // step along j
+                const int K = G::K(j), SH = G::SH(j), MK = (1 << K) - 1;
+                const int fld = (tl >> SH) & MK, nf = fld + (sj ? 1 : -1);
+                tl = (tl & ~(MK << SH)) | ((nf & MK) << SH);
+                if (nf < 0 || nf > MK) {
+                    const uint64_t unit = 1ull << ((NDIM - 1 - j) * p.bits);
+                    tk = sj ? tk + unit : tk - unit;
+                    ++carries; cdir = 2 * j + sj;
+                }
+            }
+            if (l2 >= 0) {   // step along l2
+                const int K = G::K(l2), SH = G::SH(l2), MK = (1 << K) - 1;
+                const int fld = (tl >> SH) & MK, nf = fld + (sl ? 1 : -1);
+                tl = (tl & ~(MK << SH)) | ((nf & MK) << SH);
+                if (nf < 0 || nf > MK) {
+                    const uint64_t unit = 1ull << ((NDIM - 1 - l2) * p.bits);
+                    tk = sl ? tk + unit : tk - unit;
+                    ++carries; cdir = 2 * l2 + sl;
+                }
+            }
+            const unsigned long long bit = 1ull << tl;
+            uint32_t row = NBR_NONE;
+            if (carries == 0) row = r;
+            else if (carries == 1) row = st.adj[(size_t)r * ND + cdir];
+            if (!GROW) {
+                if (row == NBR_NONE) row = ht_find(st.table, slots, tk);
+                if (row != NBR_NONE) atomicOr((unsigned long long*)&st.keep[row], bit);
+                continue;
+            }
+            // GROW. A brick that existed before this launch (row < NB0) takes the bit in its mask;
+            // a brick created during this launch collects bits in pend[slot] (folded in by link).
+            bool fresh;   // did THIS thread activate the cell?
+            if (row != NBR_NONE && row < NB0) {
+                fresh = !(atomicOr((unsigned long long*)&st.mask[row], bit) & bit);
+            } else {
+                bool inserted;
+                const uint64_t s = ht_upsert(st.table, slots, tk, inserted);
+                if (s == ~0ull) { atomicOr(&ds->err, E_TABLE_FULL); continue; }
+                if (inserted) {
+                    const uint32_t nr = atomicAdd(&ds->NB, 1u);
+                    if (nr >= p.capB) { atomicOr(&ds->err, E_CAPACITY); continue; }
+                    st.bkey[nr] = tk; st.slot_of[nr] = (uint32_t)s; st.grown[nr] = 0ull; st.mask[nr] = 0ull;
+#pragma unroll
+                    for (int d = 0; d < ND; ++d) st.adj[(size_t)nr * ND + d] = NBR_NONE;
+                    __threadfence();
+                    *reinterpret_cast<volatile unsigned long long*>(&st.table[s].y) = nr;
+                    fresh = !(atomicOr((unsigned long long*)&st.pend[s], bit) & bit);
+                } else {
+                    const uint32_t er = (uint32_t)*reinterpret_cast<volatile unsigned long long*>(&st.table[s].y);
+                    if (er != NBR_NONE && er < NB0) fresh = !(atomicOr((unsigned long long*)&st.mask[er], bit) & bit);
+                    else fresh = !(atomicOr((unsigned long long*)&st.pend[s], bit) & bit);
+                }
+            }
+            if (fresh) {   // new cell: count it, fold its CFL term into the running maximum (Eq. 8)
+                ++n_new;
+                int32_t TB[NDIM], tc[NDIM];
+                unpack<NDIM>(p, tk, TB);
+                cell_coords<NDIM>(TB, tl, tc);
+                double ul[NDIM], uu[NDIM];
+                face_velocities<NDIM, DYN>(p, tc, ul, uu);
+                smax = fmax(smax, cfl_term<NDIM>(p, ul));
+            }
+        }
+        __syncthreads();
+    }
+    if (GROW) {
+        const double nn = block_sum((double)n_new);     // exact: counts << 2^53
+        smax = block_max(smax);
+        if (threadIdx.x == 0) {
+            if (nn > 0.0) atomicAdd(&ds->N, (unsigned long long)nn);
+            if (smax > 0.0) atomicMax(&ds->smax_bits, (unsigned long long)__double_as_longlong(smax));
+        }
+    }
+}
+
+// ---- brick adjacency (here per brick instead of per cell) -------------------------
+// ALL = true: every brick (after init / import / prune); false: the bricks created by this step's
+// grow, which also take their active bits from pend[] and patch their neighbours' rows.
+template <int NDIM, bool ALL>
+__device__ void phase_link(const Params& p, const Store& st, DevState* ds) {
+    constexpr int ND = 2 * NDIM;
+    const uint32_t first = ALL ? 0u : ds->NB_before_grow;
+    const uint32_t NB = min(ds->NB, p.capB);
+    const uint64_t slots = ds->slots;
+    const uint64_t items = (uint64_t)(NB - first) * ND;
+    const uint64_t fmask = (1ull << p.bits) - 1ull;
+    for (uint64_t w = gtid(); w < items; w += gthreads()) {
+        const uint32_t row = first + (uint32_t)(w / ND);
+        const int d = (int)(w % ND), j = d >> 1;
+        const uint64_t key = st.bkey[row];
+        const int fs = (NDIM - 1 - j) * p.bits;
+        const uint64_t fld = (key >> fs) & fmask;
+        uint32_t nb = NBR_NONE;
+        if ((d & 1) ? (fld != fmask) : (fld != 0)) nb = ht_find(st.table, slots, (d & 1) ? key + (1ull << fs) : key - (1ull << fs));
+        st.adj[(size_t)row * ND + d] = nb;
+        if (!ALL) {
+            if (nb != NBR_NONE) st.adj[(size_t)nb * ND + (d ^ 1)] = row;
+            if (d == 0) {
+                const uint32_t s = st.slot_of[row];
+                st.mask[row] = st.pend[s];
+                st.pend[s] = 0ull;
+            }
+        }
+    }
+}
+
+// CFL maximum over all active cells (init / import / after a prune; grow maintains it incrementally)
+template <int NDIM, int DYN>
+__device__ void phase_smax(const Params& p, const Store& st, DevState* ds) {
+    const uint32_t NB = min(ds->NB, p.capB);
+    const uint64_t items = (uint64_t)NB * 64;
+    double smax = 0.0;
+    for (uint64_t i = gtid(); i < items; i += gthreads()) {
+        const uint32_t b = (uint32_t)(i >> 6);
+        const int l = (int)(i & 63);
+        if (!((st.mask[b] >> l) & 1ull)) continue;
+        int32_t B[NDIM], c[NDIM];
+        unpack<NDIM>(p, st.bkey[b], B);
+        cell_coords<NDIM>(B, l, c);
+        double ul[NDIM], uu[NDIM];
+        face_velocities<NDIM, DYN>(p, c, ul, uu);
+        smax = fmax(smax, cfl_term<NDIM>(p, ul));
+    }
+    smax = block_max(smax);
+    if (threadIdx.x == 0 && smax > 0.0) atomicMax(&ds->smax_bits, (unsigned long long)__double_as_longlong(smax));
+}
+
+// ---- a2+a4 pass 1: every active cell computes the fluxes of the faces it is UPWIND of -----------
+// Gather form D2 (= Eq. 7 + Alg. 1 + high-resolution term):
+//   T_l   = u+_{c,l}(P_c - P_{c-e^l}) + u-_{c+e^l,l}(P_{c+e^l} - P_c)
+//   G_j   = P*_{c,(j)} = P_c - sum_{l != j} 1/2 tau_l T_l
+//   sig_j = mc(P_c - P_{c-e^j}, P_{c+e^j} - P_c)     (limited wave when c is the upwind cell)
+//   upper face, u = u_{c+e^j,j} > 0:  F = u (G_j + 1/2 (1 - tau_j u) sig_j)
+//   lower face, u = u_{c,j}     < 0:  F = u (G_j - 1/2 (1 + tau_j u) sig_j)
+// A face whose upwind cell is NOT active carries only the high-resolution term; the active
+// downwind cell computes it (needs the two-hop value).
+// tau_j F goes to the downwind cell: through shared memory inside the brick, through phi[] across a
+// brick face (the downwind cell sets its fetch bit and picks it up in pass 2).
+// Qn <- P_c - sum_j tau_j (F_up - F_lo) over the faces resolved inside the brick.
+template <int NDIM, int DYN>
+__device__ void phase_flux1(const Params& p, const Store& st, DevState* ds) {
+    using G = Geo<NDIM>;
+    constexpr int ND = 2 * NDIM;
+    __shared__ double sQ[WPB][64];
+    __shared__ double sAcc[WPB][64];
+    __shared__ unsigned long long sFetch[WPB][ND];
+    __shared__ unsigned long long sNbMask[WPB][ND];
+    __shared__ uint32_t sNb[WPB][ND];
+    __shared__ uint8_t sList[WPB][64];
+    const uint32_t NB = min(ds->NB, p.capB);
+    const double dt = step_dt(p, ds);
+    const bool hires = p.hi_res != 0, nolim = p.limiter != 0;
+    const unsigned w = threadIdx.x >> 5, lane = lane_id();
+    const double* __restrict__ Q = st.Q;
+    double tau[NDIM];
+#pragma unroll
+    for (int j = 0; j < NDIM; ++j) tau[j] = dt / p.h[j];
+    for (uint32_t b = gwarp(); b < NB; b += gwarps()) {   // warp-uniform
+        const uint64_t m = st.mask[b];
+        if (lane < ND) {
+            const uint32_t nb = st.adj[(size_t)b * ND + lane];
+            sNb[w][lane] = nb;
+            sNbMask[w][lane] = nb != NBR_NONE ? st.mask[nb] : 0ull;
+            sFetch[w][lane] = 0ull;
+        }
+        sQ[w][lane] = Q[(size_t)b * 64 + lane];
+        sQ[w][lane + 32] = Q[(size_t)b * 64 + 32 + lane];
+        sAcc[w][lane] = 0.0;
+        sAcc[w][lane + 32] = 0.0;
+        const uint32_t m_lo = (uint32_t)m, m_hi = (uint32_t)(m >> 32);
+        const uint32_t below = (1u << lane) - 1u;
+        if ((m_lo >> lane) & 1u) sList[w][__popc(m_lo & below)] = (uint8_t)lane;
+        if ((m_hi >> lane) & 1u) sList[w][__popc(m_lo) + __popc(m_hi & below)] = (uint8_t)(lane + 32);
+        const int cnt = __popcll(m);
+        __syncwarp();
+        int32_t B[NDIM];
+        unpack<NDIM>(p, st.bkey[b], B);
+        for (int r0 = 0; r0 < cnt; r0 += 32) {             // active cells, 32 at a time
+            const bool act = r0 + (int)lane < cnt;
+            const int l = act ? sList[w][r0 + lane] : 0;
+            double q0 = 0.0, part = 0.0, S = 0.0;
+            double ul[NDIM], uu[NDIM], dm[NDIM], dp[NDIM], T[NDIM];
+            unsigned am = 0, ap = 0;                        // bit j: direct neighbour active
+            if (act) {
+                q0 = sQ[w][l];
+                int32_t c[NDIM];
+                cell_coords<NDIM>(B, l, c);
+                face_velocities<NDIM, DYN>(p, c, ul, uu);
+#pragma unroll
+                for (int j = 0; j < NDIM; ++j) {
+                    constexpr int dummy = 0; (void)dummy;
+                    const int s = 1 << G::SH(j), MK = G::MK(j);
+                    const int lj = (l >> G::SH(j)) & MK;
+                    double vm, vp;
+                    if (lj > 0) { vm = sQ[w][l - s]; am |= (unsigned)((m >> (l - s)) & 1ull) << j; }
+                    else {
+                        const uint32_t nb = sNb[w][2 * j];
+                        const int lw = l + MK * s;
+                        vm = nb != NBR_NONE ? __ldg(&Q[(size_t)nb * 64 + lw]) : 0.0;
+                        am |= (unsigned)((sNbMask[w][2 * j] >> lw) & 1ull) << j;
+                    }
+                    if (lj < MK) { vp = sQ[w][l + s]; ap |= (unsigned)((m >> (l + s)) & 1ull) << j; }
+                    else {
+                        const uint32_t nb = sNb[w][2 * j + 1];
+                        const int lw = l - MK * s;
+                        vp = nb != NBR_NONE ? __ldg(&Q[(size_t)nb * 64 + lw]) : 0.0;
+                        ap |= (unsigned)((sNbMask[w][2 * j + 1] >> lw) & 1ull) << j;
+                    }
+                    dm[j] = q0 - vm;
+                    dp[j] = vp - q0;
+                    double t = 0.0;
+                    if (ul[j] > 0.0) t = ul[j] * dm[j];
+                    if (uu[j] < 0.0) t = fma(uu[j], dp[j], t);
+                    T[j] = (0.5 * tau[j]) * t;
+                    S += T[j];
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < NDIM; ++j) {
+                const int s = 1 << G::SH(j), MK = G::MK(j);
+                int du = -1, dl = -1;         // in-brick destinations of the owned upper / lower face flux
+                double Fu = 0.0, Fl = 0.0;
+                if (act) {
+                    const int lj = (l >> G::SH(j)) & MK;
+                    const double Gj = (q0 - S) + T[j];     // P*_{c,(j)}
+                    const double sig = (hires && !nolim) ? mc_limit_fast(dm[j], dp[j]) : 0.0;
+                    const double tj = tau[j];
+                    const bool a_p = (ap >> j) & 1u, a_m = (am >> j) & 1u;
+                    {   // upper face of c
+                        const double u = uu[j];
+                        if (u > 0.0) {
+                            const double a = tj * u;
+                            const double wv = hires ? (nolim ? dp[j] : sig) : 0.0;
+                            const double F = a * fma(0.5 * (1.0 - a), wv, Gj);
+                            part -= F;
+                            if (a_p) {
+                                if (lj < MK) { du = l + s; Fu = F; }
+                                else st.phi[((size_t)b * ND + 2 * j + 1) * 32 + G::fidx(j, l)] = F;
+                            }
+                        } else if (u < 0.0) {
+                            if (a_p) {
+                                if (lj == MK) atomicOr(&sFetch[w][2 * j + 1], 1ull << l);
+                            } else if (hires) {   // upwind cell c+e^j inactive: W = 0 - P_c, W_up = P_{c+2e^j} - 0
+                                double v2;
+                                if (lj + 2 <= MK) v2 = sQ[w][l + 2 * s];
+                                else {
+                                    const uint32_t nb = sNb[w][2 * j + 1];
+                                    v2 = nb != NBR_NONE ? __ldg(&Q[(size_t)nb * 64 + (l + (1 - MK) * s)]) : 0.0;
+                                }
+                                const double wv = nolim ? -q0 : mc_limit(-q0, v2);
+                                const double a = tj * u;
+                                part -= (-0.5 * a) * (1.0 + a) * wv;
+                            }
+                        }
+                    }
+                    {   // lower face of c
+                        const double u = ul[j];
+                        if (u < 0.0) {
+                            const double a = tj * u;
+                            const double wv = hires ? (nolim ? dm[j] : sig) : 0.0;
+                            const double F = a * fma(-0.5 * (1.0 + a), wv, Gj);
+                            part += F;
+                            if (a_m) {
+                                if (lj > 0) { dl = l - s; Fl = F; }
+                                else st.phi[((size_t)b * ND + 2 * j) * 32 + G::fidx(j, l)] = F;
+                            }
+                        } else if (u > 0.0) {
+                            if (a_m) {
+                                if (lj == 0) atomicOr(&sFetch[w][2 * j], 1ull << l);
+                            } else if (hires) {   // upwind cell c-e^j inactive: W = P_c - 0, W_up = 0 - P_{c-2e^j}
+                                double v2;
+                                if (lj - 2 >= 0) v2 = sQ[w][l - 2 * s];
+                                else {
+                                    const uint32_t nb = sNb[w][2 * j];
+                                    v2 = nb != NBR_NONE ? __ldg(&Q[(size_t)nb * 64 + (l + (MK - 1) * s)]) : 0.0;
+                                }
+                                const double wv = nolim ? q0 : mc_limit(q0, -v2);
+                                const double a = tj * u;
+                                part += (0.5 * a) * (1.0 - a) * wv;
+                            }
+                        }
+                    }
+                }
+                // deliver inside the brick: for a fixed (j, side) the destinations are distinct
+                if (du >= 0) sAcc[w][du] += Fu;
+                __syncwarp();
+                if (dl >= 0) sAcc[w][dl] -= Fl;
+                __syncwarp();
+            }
+            if (act) sAcc[w][l] += q0 + part;
+            __syncwarp();
+        }
+        st.Qn[(size_t)b * 64 + lane] = sAcc[w][lane];
+        st.Qn[(size_t)b * 64 + 32 + lane] = sAcc[w][lane + 32];
+        if (lane < ND) st.fetch[(size_t)b * ND + lane] = sFetch[w][lane];
+        __syncwarp();
+    }
+}
+
+// ---- a5+a6 pass 2: fetch the fluxes owned by neighbour bricks, finish the update, sum the mass --
+template <int NDIM>
+__device__ void phase_flux2(const Params& p, const Store& st, DevState* ds) {
+    using G = Geo<NDIM>;
+    constexpr int ND = 2 * NDIM;
+    const uint32_t NB = min(ds->NB, p.capB);
+    const unsigned lane = lane_id();
+    double sum = 0.0;
+    for (uint32_t b = gwarp(); b < NB; b += gwarps()) {
+        uint32_t my_nb = NBR_NONE;
+        unsigned long long my_f = 0ull;
+        if (lane < ND) { my_nb = st.adj[(size_t)b * ND + lane]; my_f = st.fetch[(size_t)b * ND + lane]; }
+        double a0 = st.Qn[(size_t)b * 64 + lane], a1 = st.Qn[(size_t)b * 64 + 32 + lane];
+        const unsigned any = __ballot_sync(0xffffffffu, my_f != 0ull);
+        if (any) {
+#pragma unroll
+            for (int d = 0; d < ND; ++d) {
+                if (!((any >> d) & 1u)) continue;
+                const uint32_t nb = __shfl_sync(0xffffffffu, my_nb, d);
+                const unsigned long long f = __shfl_sync(0xffffffffu, my_f, d);
+                const int j = d >> 1;
+                const double* src = st.phi + ((size_t)nb * ND + (d ^ 1)) * 32;
+                if ((f >> lane) & 1ull) { const double v = src[G::fidx(j, (int)lane)]; a0 += (d & 1) ? -v : v; }
+                if ((f >> (lane + 32)) & 1ull) { const double v = src[G::fidx(j, (int)lane + 32)]; a1 += (d & 1) ? -v : v; }
+            }
+            st.Qn[(size_t)b * 64 + lane] = a0;
+            st.Qn[(size_t)b * 64 + 32 + lane] = a1;
+        }
+        sum += a0 + a1;
+    }
+    sum = block_sum(sum);
+    if (threadIdx.x == 0) st.partial[blockIdx.x] = sum;
+}
+
+// plain sum of Q and recount of the active cells (init / import / correct / prune)
+__device__ inline void phase_sum(const Params& p, const Store& st, DevState* ds, bool count) {
+    const uint32_t NB = min(ds->NB, p.capB);
+    const uint64_t items = (uint64_t)NB * 64;
+    double sum = 0.0;
+    for (uint64_t i = gtid(); i < items; i += gthreads()) sum += st.Q[i];
+    sum = block_sum(sum);
+    if (threadIdx.x == 0) st.partial[blockIdx.x] = sum;
+    if (count) {
+        double n = 0.0;
+        for (uint32_t b = gtid(); b < NB; b += gthreads()) n += (double)__popcll(st.mask[b]);
+        n = block_sum(n);
+        if (threadIdx.x == 0 && n > 0.0) atomicAdd(&ds->N, (unsigned long long)n);
+    }
+}
+
+// one block: add the partials in index order, set the scale. after_step: advance t, count.
+__device__ inline void finish_sum(const Params& p, const Store& st, DevState* ds, unsigned nparts, bool after_step) {
+    double v = 0.0;
+    for (unsigned k = threadIdx.x; k < nparts; k += blockDim.x) v += st.partial[k];
+    v = block_sum(v);
+    if (threadIdx.x == 0) {
+        ds->sumQ = v;
+        if (!(v > 0.0) || !isfinite(v)) {
+            if (p.normalise || !isfinite(v)) atomicOr(&ds->err, E_DEGENERATE);
+        }
+        const double old = ds->scale;
+        ds->mass = v * old;
+        if (p.normalise && v > 0.0) ds->scale = 1.0 / v;
+        if (ds->N > p.max_cells) atomicOr(&ds->err, E_CAPACITY);
+        if (after_step) {
+            const double dt = step_dt(p, ds);
+            if (!(dt > 0.0)) atomicOr(&ds->err, E_DEGENERATE);
+            ds->dt = dt;
+            ds->t += dt;
+            ds->steps += 1;
+            ds->cell_updates += ds->N;
+            ds->inserted_total += ds->N - ds->N_before_grow;
+        }
+    }
+}
+
+// ---- a7 prune, D3 (Alg. 3) -------------------------------------------
+// mark = phase_targets<.., false>. Then: new mask = mask & keep; bricks left without a cell are
+// freed; surviving bricks are stream-compacted (decoupled-lookback scan over BRICKS), removed cells
+// are zeroed, the table is rebuilt and the adjacency re-linked.
+__device__ inline void phase_prune_scan(const Params& p, const Store& st, DevState* ds) {
+    const uint32_t NB = min(ds->NB, p.capB);
+    if (NB == 0) { if (gtid() == 0) ds->NB_after_prune = 0; return; }
+    scan_compact(
+        NB, st.tile_state, &ds->tile_counter, &ds->NB_after_prune,
+        [&](uint32_t i) { return (st.mask[i] & st.keep[i]) != 0ull; },
+        [&](uint32_t i, uint32_t d) {
+            st.newrow[i] = d;
+            st.bkey2[d] = st.bkey[i];
+            st.mask2[d] = st.mask[i] & st.keep[i];
+        },
+        [&](uint32_t i) { st.newrow[i] = NBR_NONE; });
+}
+
+// move the surviving bricks' rows (Q -> Qn at the new row), zero removed cells, keep the GROWN bit
+// only for cells still >= p* (their targets were all kept)
+__device__ inline void phase_prune_move(const Params& p, const Store& st, DevState* ds) {
+    const uint32_t NB = min(ds->NB, p.capB);
+    const double scale = ds->scale, thresh = p.thresh;
+    const unsigned lane = lane_id();
+    for (uint32_t b = gwarp(); b < NB; b += gwarps()) {
+        const uint32_t d = st.newrow[b];
+        if (d == NBR_NONE) continue;
+        const uint64_t nm = st.mask[b] & st.keep[b];
+        double q0 = st.Q[(size_t)b * 64 + lane], q1 = st.Q[(size_t)b * 64 + 32 + lane];
+        if (!((nm >> lane) & 1ull)) q0 = 0.0;
+        if (!((nm >> (lane + 32)) & 1ull)) q1 = 0.0;
+        st.Qn[(size_t)d * 64 + lane] = q0;
+        st.Qn[(size_t)d * 64 + 32 + lane] = q1;
+        const uint64_t ge = (uint64_t)__ballot_sync(0xffffffffu, scale * q0 >= thresh) |
+                            ((uint64_t)__ballot_sync(0xffffffffu, scale * q1 >= thresh) << 32);
+        if (lane == 0) st.grown2[d] = st.grown[b] & ge & nm;
+    }
+}
+
+// rows [NB_after_prune, NB) of both value buffers go back to zero (invariant: unused rows are zero)
+__device__ inline void phase_zero_tail(const Params& p, const Store& st, DevState* ds) {
+    const uint64_t first = (uint64_t)ds->NB_after_prune * 64, last = (uint64_t)min(ds->NB, p.capB) * 64;
+    for (uint64_t i = first + gtid(); i < last; i += gthreads()) { st.Q[i] = 0.0; st.Qn[i] = 0.0; }
+}
+
+// clear the active part of the table (ds->slots was set for the new brick count)
+__device__ inline void phase_clear_table(const Store& st, const DevState* ds) {
+    const uint64_t slots = ds->slots;
+    const ulonglong2 e = make_ulonglong2(KEY_EMPTY, KEY_EMPTY);
+    for (uint64_t s = gtid(); s < slots; s += gthreads()) { st.table[s] = e; st.pend[s] = 0ull; }
+}
+
+// insert every brick key with its row (table was cleared)
+__device__ inline void phase_rebuild(const Params& p, const Store& st, DevState* ds) {
+    const uint32_t NB = min(ds->NB, p.capB);
+    const uint64_t slots = ds->slots;
+    for (uint32_t i = gtid(); i < NB; i += gthreads()) {
+        const uint64_t s = ht_claim(st.table, slots, st.bkey[i]);
+        if (s >= ~0ull - 1) { atomicOr(&ds->err, s == ~0ull ? E_DEGENERATE : E_TABLE_FULL); continue; }  // duplicate key
+        st.table[s].y = i;
+    }
+}
+
+// ---- D5 / A8 init_gaussian: one thread per candidate cell of the ellipsoid's bounding box ---------
+struct GaussArgs {
+    double inv[MAXN * MAXN];   // Sigma^-1 (or R^-1 for correct)
+    double v[MAXN];            // correct: measurement z
+    double norm;               // P~ at the mean
+    int64_t R[MAXN];           // half-extents of the bounding box in cells
+    unsigned long long total;  // prod (2 R_j + 1)
+};
+
+template <int NDIM>
+__device__ __forceinline__ double quad_form(const double* inv, const double d[NDIM]) {
+    double q = 0.0;
+#pragma unroll
+    for (int i = 0; i < NDIM; ++i) {
+        double r = 0.0;
+#pragma unroll
+        for (int j = 0; j < NDIM; ++j) r += inv[i * NDIM + j] * d[j];
+        q += d[i] * r;
+    }
+    return q;
+}
+
+// create the brick of cell c if absent (claim + row allocation + publication). Used by init / import,
+// which run the claim pass and the fill pass as separate launches.
+template <int NDIM>
+__device__ __forceinline__ void claim_brick(const Params& p, const Store& st, DevState* ds, const int32_t c[NDIM]) {
+    constexpr int ND = 2 * NDIM;
+    int32_t B[NDIM];
+    cell_to_brick<NDIM>(c, B);
+    const uint64_t bk = pack<NDIM>(p, B);
+    bool inserted;
+    const uint64_t s = ht_upsert(st.table, ds->slots, bk, inserted);
+    if (s == ~0ull) { atomicOr(&ds->err, E_TABLE_FULL); return; }
+    if (!inserted) return;
+    const uint32_t nr = atomicAdd(&ds->NB, 1u);
+    if (nr >= p.capB) { atomicOr(&ds->err, E_CAPACITY); return; }
+    st.bkey[nr] = bk; st.grown[nr] = 0ull; st.mask[nr] = 0ull;
+#pragma unroll
+    for (int d = 0; d < ND; ++d) st.adj[(size_t)nr * ND + d] = NBR_NONE;
+    st.table[s].y = nr;
+}
+// second pass: activate cell c with stored mass q (its brick exists)
+template <int NDIM>
+__device__ __forceinline__ void fill_cell(const Params& p, const Store& st, DevState* ds, const int32_t c[NDIM], double q) {
+    int32_t B[NDIM];
+    const int l = cell_to_brick<NDIM>(c, B);
+    const uint32_t row = ht_find(st.table, ds->slots, pack<NDIM>(p, B));
+    if (row == NBR_NONE || row >= p.capB) return;     // capacity error already recorded by the claim pass
+    const unsigned long long bit = 1ull << l;
+    if (atomicOr((unsigned long long*)&st.mask[row], bit) & bit) { atomicOr(&ds->err, E_DEGENERATE); return; }  // duplicate key
+    st.Q[(size_t)row * 64 + l] = q;
+}
+
+template <int NDIM, bool FILL>
+__device__ void phase_init_gaussian(const Params& p, const Store& st, DevState* ds, const GaussArgs& g) {
+    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+    for (unsigned long long r = gtid(); r < g.total; r += stride) {
+        int32_t c[NDIM];
+        unsigned long long rem = r;
+#pragma unroll
+        for (int j = NDIM - 1; j >= 0; --j) {
+            const unsigned long long wd = 2ull * g.R[j] + 1ull;
+            c[j] = (int32_t)((long long)(rem % wd) - g.R[j]);
+            rem /= wd;
+        }
+        double d[NDIM];
+#pragma unroll
+        for (int j = 0; j < NDIM; ++j) d[j] = (double)c[j] * p.h[j];
+        const double val = exp(-0.5 * quad_form<NDIM>(g.inv, d)) * g.norm;
+        if (!(val >= p.thresh)) continue;
+        bool ok = true;
+#pragma unroll
+        for (int j = 0; j < NDIM; ++j) ok = ok && c[j] >= -p.bias && c[j] <= p.bias - 1;
+        if (!ok) { atomicOr(&ds->err, E_KEY_RANGE); continue; }
+        if (FILL) fill_cell<NDIM>(p, st, ds, c, val);
+        else claim_brick<NDIM>(p, st, ds, c);
+    }
+}
+
+template <int NDIM, bool FILL>
+__device__ void phase_import(const Params& p, const Store& st, DevState* ds, const int32_t* keys,
+                             const double* vals, uint64_t count) {
+    for (uint64_t i = gtid(); i < count; i += gthreads()) {
+        int32_t c[NDIM];
+        bool ok = true;
+#pragma unroll
+        for (int j = 0; j < NDIM; ++j) {
+            c[j] = keys[(size_t)i * NDIM + j];
+            ok = ok && c[j] >= -p.bias && c[j] <= p.bias - 1;
+        }
+        if (!ok) { atomicOr(&ds->err, E_KEY_RANGE); continue; }
+        if (FILL) fill_cell<NDIM>(p, st, ds, c, vals[i]);
+        else claim_brick<NDIM>(p, st, ds, c);
+    }
+}
+
+// ---- a8 correct, D4 / Eq. (4): Q_c *= exp(-1/2 (z - x_c)^T R^-1 (z - x_c)) ------------
+template <int NDIM>
+__device__ void phase_correct(const Params& p, const Store& st, DevState* ds, const GaussArgs& g) {
+    const uint32_t NB = min(ds->NB, p.capB);
+    const uint64_t items = (uint64_t)NB * 64;
+    for (uint64_t i = gtid(); i < items; i += gthreads()) {
+        const uint32_t b = (uint32_t)(i >> 6);
+        const int l = (int)(i & 63);
+        if (!((st.mask[b] >> l) & 1ull)) continue;
+        int32_t B[NDIM], c[NDIM];
+        unpack<NDIM>(p, st.bkey[b], B);
+        cell_coords<NDIM>(B, l, c);
+        double d[NDIM];
+#pragma unroll
+        for (int j = 0; j < NDIM; ++j) d[j] = g.v[j] - (p.mu[j] + (double)c[j] * p.h[j]);
+        st.Q[i] *= exp(-0.5 * quad_form<NDIM>(g.inv, d));
+    }
+}
+
+// export: a warp reserves popc(mask) output rows per brick (order of bricks is unspecified)
+template <int NDIM>
+__device__ void phase_export(const Params& p, const Store& st, DevState* ds, int32_t* keys, double* out) {
+    const uint32_t NB = min(ds->NB, p.capB);
+    const double scale = ds->scale;
+    const unsigned lane = lane_id();
+    for (uint32_t b = gwarp(); b < NB; b += gwarps()) {
+        const uint64_t m = st.mask[b];
+        const int cnt = __popcll(m);
+        if (cnt == 0) continue;
+        unsigned base = 0;
+        if (lane == 0) base = atomicAdd(&ds->export_count, (unsigned)cnt);
+        base = __shfl_sync(0xffffffffu, base, 0);
+        int32_t B[NDIM];
+        unpack<NDIM>(p, st.bkey[b], B);
+#pragma unroll
+        for (int hh = 0; hh < 2; ++hh) {
+            const int l = (int)lane + 32 * hh;
+            if (!((m >> l) & 1ull)) continue;
+            const size_t o = base + (unsigned)__popcll(m & ((1ull << l) - 1ull));
+            if (keys) {
+                int32_t c[NDIM];
+                cell_coords<NDIM>(B, l, c);
+#pragma unroll
+                for (int j = 0; j < NDIM; ++j) keys[o * NDIM + j] = c[j];
+            }
+            if (out) out[o] = scale * st.Q[(size_t)b * 64 + l];
+        }
+    }
+}
+
+}  // namespace gbees

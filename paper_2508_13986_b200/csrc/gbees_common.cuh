@@ -8,9 +8,7 @@ namespace gbees {
 
 constexpr int MAXN = 6;
 constexpr uint64_t KEY_EMPTY = ~0ull;            // all-ones is never a packed key (A18)
-constexpr uint64_t KEY_GROWN = 1ull << 63;       // pool-only flag: Targets(c) already inserted
 constexpr uint32_t NBR_NONE = 0xFFFFFFFFu;       // no neighbour, direct or two-hop
-constexpr uint32_t NBR_TAG = 0x80000000u;        // direct neighbour missing; low bits = two-hop cell
 
 enum ErrBits : int { E_CAPACITY = 1, E_KEY_RANGE = 2, E_DEGENERATE = 4, E_TABLE_FULL = 8 };
 
@@ -22,56 +20,65 @@ struct Params {
     int hi_res;
     int limiter;
     int normalise;
-    int64_t bias;        // 2^(bits-1)
+    int64_t bias;        // 2^(bits-1): cell coordinates live in [-bias, bias-1] (A18)
     double h[MAXN];
     double mu[MAXN];     // grid origin
     double par[MAXN * MAXN];
     double thresh;
     double cfl;
-    uint32_t cap;        // pool capacity (cells)
-    uint64_t slots;      // hashtable slots allocated (= ceil(cap / load_factor))
-    double load_factor;  // rehash to a larger active table when N / slots_in_use exceeds this
+    uint64_t max_cells;  // opts.max_cells: active-cell capacity
+    uint32_t capB;       // brick capacity (rows of 64 cell slots)
+    uint64_t slots;      // hashtable slots allocated (= ceil(capB / load_factor))
+    double load_factor;  // rehash to a larger active table when NB / slots_in_use exceeds this
 };
 
 // Mutable scalars living in device memory (one struct, read back after each API call).
 struct DevState {
-    uint32_t N;                 // active cells
-    uint32_t N_before_grow;     // cells before this step's grow (link range start)
+    unsigned long long N;          // active cells
+    unsigned long long N_before_grow;
+    uint32_t NB;                   // bricks in use (rows 0..NB-1)
+    uint32_t NB_before_grow;       // bricks before this step's grow (link range start)
     int err;
-    unsigned int ticket;        // last-block election for the sum reduction
+    unsigned int ticket;           // last-block election for the sum reduction
     unsigned long long smax_bits;  // bits of max_c sum_j |u_cj|/h_j  (>= 0, so uint order == fp order)
-    double sumQ;                // sum of stored masses Q
-    double scale;               // P = scale * Q
+    double sumQ;                   // sum of stored masses Q
+    double scale;                  // P = scale * Q
     double dt;
-    double dt_cap;              // caller's cap for this step (<= 0 / non-finite: none)
+    double dt_cap;                 // caller's cap for this step (<= 0 / non-finite: none)
     double t;
-    double mass;                // pre-normalisation mass of the last step (in normalised units)
+    double mass;                   // pre-normalisation mass of the last step (in normalised units)
     unsigned long long steps;
     unsigned long long cell_updates;
-    unsigned int tile_counter;  // dynamic tile ids for the decoupled-lookback scan
-    uint32_t N_after_prune;
+    unsigned int tile_counter;     // dynamic tile ids for the decoupled-lookback scan
+    uint32_t NB_after_prune;
     unsigned long long inserted_total;   // cells created by grow since init
     unsigned long long prune_scanned;    // sum over prunes of the cell count scanned
     unsigned long long prunes;
-    unsigned int parity;                 // toggled by every prune inside the persistent loop (buffer swap)
-    unsigned int pad_;
+    unsigned int parity;                 // persistent loop: bit 0 = Q/Qn swapped, bit 1 = metadata buffers swapped
+    unsigned int export_count;           // export: next output row
     unsigned long long phase_ns[12];     // persistent loop: device-timer ns per phase (index = GBEES_PH_*)
     unsigned long long slots;            // hashtable slots in use (<= Params::slots), resized at rehash
 };
 
-struct Pool {
-    uint64_t* key;       // [cap] packed key | KEY_GROWN
-    double* Q;           // [cap] stored mass (P = scale * Q)
-    double* acc;         // [cap] pass-A partial update
-    uint16_t* mask;      // [cap] which face fluxes pass B must gather (bit j: lower, bit 8+j: upper)
-    uint32_t* nbr;       // [2n][cap] adjacency: dir d = 2j (lower, -e^j), 2j+1 (upper, +e^j)
-    double* phi;         // [2n][cap] tau_j * face flux computed by the upwind owner: 2j -> lower face, 2j+1 -> upper face
-    ulonglong2* table;   // [slots] {key, pool index}
-    uint64_t* key2;      // compaction double buffers
-    double* Q2;
-    uint8_t* keep;       // [cap]
-    uint32_t* nbr2;      // [2n][cap] adjacency double buffer (remapped at prune)
-    uint32_t* newidx;    // [cap] old row -> new row of the last compaction (NBR_NONE = pruned)
+// Brick store. A brick is a dense box of 64 cell slots (2^K_j cells along
+// dimension j, sum K_j = 6); row r of the store holds brick r. Inactive slots hold Q = 0.
+struct Store {
+    double* Q;           // [capB][64] stored mass (P = scale * Q)
+    double* Qn;          // [capB][64] next-step buffer (pass 1 partial update, pass 2 final)
+    double* phi;         // [capB][2n][32] tau_j * flux through the EXTERNAL faces owned (upwind) by this brick
+    uint64_t* bkey;      // [capB] packed brick coordinates
+    uint64_t* mask;      // [capB] active-cell bits (bit = local index)
+    uint64_t* grown;     // [capB] cells whose Targets(c) have been inserted (autonomous f: grow once)
+    uint64_t* keep;      // [capB] prune marks
+    uint64_t* fetch;     // [capB][2n] cells that must fetch an external inflow flux in pass 2
+    uint32_t* adj;       // [capB][2n] neighbour brick rows: d = 2j (-e^j), 2j+1 (+e^j); NBR_NONE if absent
+    uint32_t* slot_of;   // [capB] hashtable slot of a brick created by this step's grow
+    ulonglong2* table;   // [slots] {brick key, row}
+    uint64_t* pend;      // [slots] active bits set in bricks created during the running grow
+    uint64_t* bkey2;     // compaction double buffers
+    uint64_t* mask2;
+    uint64_t* grown2;
+    uint32_t* newrow;    // [capB] old row -> new row of the last compaction (NBR_NONE = freed)
     unsigned long long* tile_state;  // scan descriptors
     double* partial;     // block partial sums
 };
@@ -118,6 +125,25 @@ __device__ __forceinline__ uint32_t ht_find(const ulonglong2* __restrict__ table
         if (e.x == KEY_EMPTY) { if (probes) *probes += np; return NBR_NONE; }
         if (++s == slots) s = 0;
     }
+}
+
+// Find-or-insert for kernels that mutate the table while others probe it (grow): volatile probes.
+// Returns the slot holding `key` (inserted = true if THIS thread claimed it and must publish the
+// value), or ~0ull if the table is full.
+__device__ __forceinline__ uint64_t ht_upsert(ulonglong2* table, uint64_t slots, uint64_t key, bool& inserted) {
+    uint64_t s = home_slot(key, slots);
+    inserted = false;
+    for (uint64_t tries = 0; tries < slots; ++tries) {
+        unsigned long long* kp = reinterpret_cast<unsigned long long*>(&table[s].x);
+        unsigned long long cur = *reinterpret_cast<volatile unsigned long long*>(kp);
+        if (cur == KEY_EMPTY) {
+            cur = atomicCAS(kp, KEY_EMPTY, key);
+            if (cur == KEY_EMPTY) { inserted = true; return s; }
+        }
+        if (cur == key) return s;
+        if (++s == slots) s = 0;
+    }
+    return ~0ull;
 }
 
 // Claim a slot for `key` if absent. Returns the slot index if THIS thread inserted (caller then
@@ -195,11 +221,11 @@ __device__ __forceinline__ double cfl_term(const Params& p, const double ul[NDIM
 }
 
 // monotonised-central limiter, division-free (A3)
-// active table size for N cells: room for the grid to grow 4x before the load factor is reached
-// (a 6-D blob can grow ~2-3x in one step), never below 2^20 slots, never above the allocation
-__host__ __device__ __forceinline__ unsigned long long table_slots_for(const Params& p, unsigned long long N) {
-    unsigned long long want = (unsigned long long)((double)N * 4.0 / p.load_factor) + 1ull;
-    if (want < (1ull << 20)) want = 1ull << 20;
+// active table size for NB bricks: room for the brick count to grow 4x before the load factor is
+// reached, never below 2^16 slots, never above the allocation
+__host__ __device__ __forceinline__ unsigned long long table_slots_for(const Params& p, unsigned long long NB) {
+    unsigned long long want = (unsigned long long)((double)NB * 4.0 / p.load_factor) + 1ull;
+    if (want < (1ull << 16)) want = 1ull << 16;
     return want < p.slots ? want : p.slots;
 }
 

@@ -3,7 +3,7 @@
 #include <cstdio>
 
 #include "../../include/gbees.h"
-#include "gbees_kernels.cuh"
+#include "gbees_prims.cuh"
 
 using namespace gbees;
 
@@ -130,7 +130,7 @@ int gbees_ht_lookup(gbees_ht* h, const uint64_t* q, int64_t k, uint32_t* out, ui
 }
 
 int gbees_ht_compact(gbees_ht* h, uint64_t* keys, const uint8_t* del, int64_t k, int64_t* k_out) {
-    if (!h || !keys || !del || k < 0 || k >= (int64_t)NBR_TAG) return GBEES_ERR_ARG;
+    if (!h || !keys || !del || k < 0 || k >= (int64_t)0x80000000u) return GBEES_ERR_ARG;
     HT_CU(cudaSetDevice(h->device));
     const int64_t tiles = (k + SCAN_TILE - 1) / SCAN_TILE + 1;
     if (k > h->keys2_cap) { cudaFree(h->keys2); HT_CU(cudaMalloc((void**)&h->keys2, (size_t)k * 8)); h->keys2_cap = k; }
