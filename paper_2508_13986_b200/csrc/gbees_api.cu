@@ -355,7 +355,7 @@ int gbees_create(gbees_ctx** out, int n, const double* dx, double threshold, int
     c->stage_bytes = cb * nd * 32 * 8;
     if (alloc((void**)&st.Q, cb * 512) || alloc((void**)&st.Qn, cb * 512) || alloc((void**)&st.phi, c->stage_bytes) ||
         alloc((void**)&st.bkey, cb * 8) || alloc((void**)&st.mask, cb * 8) || alloc((void**)&st.grown, cb * 8) ||
-        alloc((void**)&st.keep, cb * 8) || alloc((void**)&st.fetch, cb * nd * 8) || alloc((void**)&st.adj, cb * nd * 4) ||
+        alloc((void**)&st.keep, cb * 8) || alloc((void**)&st.fetch, cb * 64 * 2) || alloc((void**)&st.adj, cb * nd * 4) ||
         alloc((void**)&st.slot_of, cb * 4) || alloc((void**)&st.table, p.slots * sizeof(ulonglong2)) ||
         alloc((void**)&st.pend, p.slots * 8) || alloc((void**)&st.bkey2, cb * 8) || alloc((void**)&st.mask2, cb * 8) ||
         alloc((void**)&st.grown2, cb * 8) || alloc((void**)&st.newrow, cb * 4) ||
@@ -465,7 +465,12 @@ int gbees_step(gbees_ctx* c, double* dt) {
         });
         if (!c->no_grow)
             phase(c, GBEES_PH_LINK, 1, [&] { k_link<NN, false><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st); });
-        phase(c, GBEES_PH_PASSA, 1, [&] { k_flux1<NN, DD><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st); });
+        phase(c, GBEES_PH_PASSA, 1, [&] {
+            constexpr size_t smem = sizeof(Flux1Smem<NN>) * WPB;
+            static bool attr_set = false;
+            if (!attr_set) { cudaFuncSetAttribute(k_flux1<NN, DD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_set = true; }
+            k_flux1<NN, DD><<<c->grid, TPB, smem, c->stream>>>(c->p, c->st, c->d_st);
+        });
         phase(c, GBEES_PH_PASSB, 2, [&] {
             k_flux2<NN><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
             k_finish<<<1, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, c->grid, 0);

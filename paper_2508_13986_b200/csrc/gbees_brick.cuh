@@ -9,6 +9,7 @@
 // shared memory, values across a brick face from the neighbour brick's row (coalesced 8-byte loads
 // of a contiguous 512-byte row), so the per-cell adjacency and per-cell keys of a cell list are gone.
 #pragma once
+#include <cuda_pipeline.h>
 #include "gbees_prims.cuh"
 
 namespace gbees {
@@ -299,52 +300,77 @@ __device__ void phase_smax(const Params& p, const Store& st, DevState* ds) {
 // tau_j F goes to the downwind cell: through shared memory inside the brick, through phi[] across a
 // brick face (the downwind cell sets its fetch bit and picks it up in pass 2).
 // Qn <- P_c - sum_j tau_j (F_up - F_lo) over the faces resolved inside the brick.
+// Shared memory of one warp in pass 1: the brick's own row and its 2n neighbour rows (values and
+// activity flags), the update accumulator, the per-cell fetch flags and the list of active slots.
+template <int NDIM>
+struct Flux1Smem {
+    static constexpr int ROWS = 2 * NDIM + 1, OWN = 2 * NDIM;
+    double R[ROWS][64];
+    double acc[64];
+    uint16_t fl[64];
+    uint8_t A[ROWS][64];
+    uint8_t list[64];
+};
+
 template <int NDIM, int DYN>
 __device__ void phase_flux1(const Params& p, const Store& st, DevState* ds) {
     using G = Geo<NDIM>;
-    constexpr int ND = 2 * NDIM;
-    __shared__ double sQ[WPB][64];
-    __shared__ double sAcc[WPB][64];
-    __shared__ unsigned long long sFetch[WPB][ND];
-    __shared__ unsigned long long sNbMask[WPB][ND];
-    __shared__ uint32_t sNb[WPB][ND];
-    __shared__ uint8_t sList[WPB][64];
+    using SM = Flux1Smem<NDIM>;
+    constexpr int ND = 2 * NDIM, OWN = SM::OWN;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const unsigned w = threadIdx.x >> 5, lane = lane_id();
+    SM& sm = reinterpret_cast<SM*>(smem_raw)[w];
     const uint32_t NB = min(ds->NB, p.capB);
     const double dt = step_dt(p, ds);
     const bool hires = p.hi_res != 0, nolim = p.limiter != 0;
-    const unsigned w = threadIdx.x >> 5, lane = lane_id();
     const double* __restrict__ Q = st.Q;
     double tau[NDIM];
 #pragma unroll
     for (int j = 0; j < NDIM; ++j) tau[j] = dt / p.h[j];
     for (uint32_t b = gwarp(); b < NB; b += gwarps()) {   // warp-uniform
-        const uint64_t m = st.mask[b];
-        if (lane < ND) {
-            const uint32_t nb = st.adj[(size_t)b * ND + lane];
-            sNb[w][lane] = nb;
-            sNbMask[w][lane] = nb != NBR_NONE ? st.mask[nb] : 0ull;
-            sFetch[w][lane] = 0ull;
+        // ---- stage the 2n+1 rows (coalesced 256-byte loads) and their activity flags
+        uint32_t my_row = NBR_NONE;
+        uint64_t my_mask = 0ull;
+        if (lane < ND) my_row = st.adj[(size_t)b * ND + lane];
+        if (lane == OWN) my_row = b;
+        if (my_row != NBR_NONE) my_mask = st.mask[my_row];
+        const uint64_t bk = st.bkey[b];
+        uint64_t m = 0ull;
+#pragma unroll
+        for (int r = 0; r < SM::ROWS; ++r) {
+            const uint32_t row = __shfl_sync(0xffffffffu, my_row, r);
+            const uint32_t mlo = __shfl_sync(0xffffffffu, (uint32_t)my_mask, r);
+            const uint32_t mhi = __shfl_sync(0xffffffffu, (uint32_t)(my_mask >> 32), r);
+            // global -> shared without a register round trip (LDGSTS, 16 bytes per lane = one row)
+            if (row != NBR_NONE) __pipeline_memcpy_async(&sm.R[r][2 * lane], &Q[(size_t)row * 64 + 2 * lane], 16);
+            else *reinterpret_cast<double2*>(&sm.R[r][2 * lane]) = make_double2(0.0, 0.0);
+            sm.A[r][lane] = (uint8_t)((mlo >> lane) & 1u);
+            sm.A[r][lane + 32] = (uint8_t)((mhi >> lane) & 1u);
+            if (r == OWN) m = ((uint64_t)mhi << 32) | mlo;
         }
-        sQ[w][lane] = Q[(size_t)b * 64 + lane];
-        sQ[w][lane + 32] = Q[(size_t)b * 64 + 32 + lane];
-        sAcc[w][lane] = 0.0;
-        sAcc[w][lane + 32] = 0.0;
+        __pipeline_commit();
+        sm.acc[lane] = 0.0; sm.acc[lane + 32] = 0.0;
+        sm.fl[lane] = 0; sm.fl[lane + 32] = 0;
         const uint32_t m_lo = (uint32_t)m, m_hi = (uint32_t)(m >> 32);
         const uint32_t below = (1u << lane) - 1u;
-        if ((m_lo >> lane) & 1u) sList[w][__popc(m_lo & below)] = (uint8_t)lane;
-        if ((m_hi >> lane) & 1u) sList[w][__popc(m_lo) + __popc(m_hi & below)] = (uint8_t)(lane + 32);
+        if ((m_lo >> lane) & 1u) sm.list[__popc(m_lo & below)] = (uint8_t)lane;
+        if ((m_hi >> lane) & 1u) sm.list[__popc(m_lo) + __popc(m_hi & below)] = (uint8_t)(lane + 32);
         const int cnt = __popcll(m);
-        __syncwarp();
         int32_t B[NDIM];
-        unpack<NDIM>(p, st.bkey[b], B);
+        unpack<NDIM>(p, bk, B);
+        __pipeline_wait_prior(0);
+        __syncwarp();
+        const double* Rf = &sm.R[0][0];
+        const uint8_t* Af = &sm.A[0][0];
         for (int r0 = 0; r0 < cnt; r0 += 32) {             // active cells, 32 at a time
             const bool act = r0 + (int)lane < cnt;
-            const int l = act ? sList[w][r0 + lane] : 0;
+            const int l = act ? sm.list[r0 + lane] : 0;
             double q0 = 0.0, part = 0.0, S = 0.0;
             double ul[NDIM], uu[NDIM], dm[NDIM], dp[NDIM], T[NDIM];
             unsigned am = 0, ap = 0;                        // bit j: direct neighbour active
+            unsigned fl = 0;                                // bit d: fetch the flux of external face d in pass 2
             if (act) {
-                q0 = sQ[w][l];
+                q0 = sm.R[OWN][l];
                 int32_t c[NDIM];
                 cell_coords<NDIM>(B, l, c);
                 face_velocities<NDIM, DYN>(p, c, ul, uu);
@@ -353,21 +379,11 @@ __device__ void phase_flux1(const Params& p, const Store& st, DevState* ds) {
                     constexpr int dummy = 0; (void)dummy;
                     const int s = 1 << G::SH(j), MK = G::MK(j);
                     const int lj = (l >> G::SH(j)) & MK;
-                    double vm, vp;
-                    if (lj > 0) { vm = sQ[w][l - s]; am |= (unsigned)((m >> (l - s)) & 1ull) << j; }
-                    else {
-                        const uint32_t nb = sNb[w][2 * j];
-                        const int lw = l + MK * s;
-                        vm = nb != NBR_NONE ? __ldg(&Q[(size_t)nb * 64 + lw]) : 0.0;
-                        am |= (unsigned)((sNbMask[w][2 * j] >> lw) & 1ull) << j;
-                    }
-                    if (lj < MK) { vp = sQ[w][l + s]; ap |= (unsigned)((m >> (l + s)) & 1ull) << j; }
-                    else {
-                        const uint32_t nb = sNb[w][2 * j + 1];
-                        const int lw = l - MK * s;
-                        vp = nb != NBR_NONE ? __ldg(&Q[(size_t)nb * 64 + lw]) : 0.0;
-                        ap |= (unsigned)((sNbMask[w][2 * j + 1] >> lw) & 1ull) << j;
-                    }
+                    const int im = lj > 0 ? OWN * 64 + l - s : (2 * j) * 64 + l + MK * s;
+                    const int ip = lj < MK ? OWN * 64 + l + s : (2 * j + 1) * 64 + l - MK * s;
+                    const double vm = Rf[im], vp = Rf[ip];
+                    am |= (unsigned)Af[im] << j;
+                    ap |= (unsigned)Af[ip] << j;
                     dm[j] = q0 - vm;
                     dp[j] = vp - q0;
                     double t = 0.0;
@@ -401,15 +417,10 @@ __device__ void phase_flux1(const Params& p, const Store& st, DevState* ds) {
                             }
                         } else if (u < 0.0) {
                             if (a_p) {
-                                if (lj == MK) atomicOr(&sFetch[w][2 * j + 1], 1ull << l);
+                                if (lj == MK) fl |= 1u << (2 * j + 1);
                             } else if (hires) {   // upwind cell c+e^j inactive: W = 0 - P_c, W_up = P_{c+2e^j} - 0
-                                double v2;
-                                if (lj + 2 <= MK) v2 = sQ[w][l + 2 * s];
-                                else {
-                                    const uint32_t nb = sNb[w][2 * j + 1];
-                                    v2 = nb != NBR_NONE ? __ldg(&Q[(size_t)nb * 64 + (l + (1 - MK) * s)]) : 0.0;
-                                }
-                                const double wv = nolim ? -q0 : mc_limit(-q0, v2);
+                                const int i2 = lj + 2 <= MK ? OWN * 64 + l + 2 * s : (2 * j + 1) * 64 + l + (1 - MK) * s;
+                                const double wv = nolim ? -q0 : mc_limit(-q0, Rf[i2]);
                                 const double a = tj * u;
                                 part -= (-0.5 * a) * (1.0 + a) * wv;
                             }
@@ -428,15 +439,10 @@ __device__ void phase_flux1(const Params& p, const Store& st, DevState* ds) {
                             }
                         } else if (u > 0.0) {
                             if (a_m) {
-                                if (lj == 0) atomicOr(&sFetch[w][2 * j], 1ull << l);
+                                if (lj == 0) fl |= 1u << (2 * j);
                             } else if (hires) {   // upwind cell c-e^j inactive: W = P_c - 0, W_up = 0 - P_{c-2e^j}
-                                double v2;
-                                if (lj - 2 >= 0) v2 = sQ[w][l - 2 * s];
-                                else {
-                                    const uint32_t nb = sNb[w][2 * j];
-                                    v2 = nb != NBR_NONE ? __ldg(&Q[(size_t)nb * 64 + (l + (MK - 1) * s)]) : 0.0;
-                                }
-                                const double wv = nolim ? q0 : mc_limit(q0, -v2);
+                                const int i2 = lj - 2 >= 0 ? OWN * 64 + l - 2 * s : (2 * j) * 64 + l + (MK - 1) * s;
+                                const double wv = nolim ? q0 : mc_limit(q0, -Rf[i2]);
                                 const double a = tj * u;
                                 part += (0.5 * a) * (1.0 - a) * wv;
                             }
@@ -444,17 +450,18 @@ __device__ void phase_flux1(const Params& p, const Store& st, DevState* ds) {
                     }
                 }
                 // deliver inside the brick: for a fixed (j, side) the destinations are distinct
-                if (du >= 0) sAcc[w][du] += Fu;
+                if (du >= 0) sm.acc[du] += Fu;
                 __syncwarp();
-                if (dl >= 0) sAcc[w][dl] -= Fl;
+                if (dl >= 0) sm.acc[dl] -= Fl;
                 __syncwarp();
             }
-            if (act) sAcc[w][l] += q0 + part;
+            if (act) { sm.acc[l] += q0 + part; sm.fl[l] = (uint16_t)fl; }
             __syncwarp();
         }
-        st.Qn[(size_t)b * 64 + lane] = sAcc[w][lane];
-        st.Qn[(size_t)b * 64 + 32 + lane] = sAcc[w][lane + 32];
-        if (lane < ND) st.fetch[(size_t)b * ND + lane] = sFetch[w][lane];
+        st.Qn[(size_t)b * 64 + lane] = sm.acc[lane];
+        st.Qn[(size_t)b * 64 + 32 + lane] = sm.acc[lane + 32];
+        st.fetch[(size_t)b * 64 + lane] = sm.fl[lane];
+        st.fetch[(size_t)b * 64 + 32 + lane] = sm.fl[lane + 32];
         __syncwarp();
     }
 }
@@ -469,20 +476,21 @@ __device__ void phase_flux2(const Params& p, const Store& st, DevState* ds) {
     double sum = 0.0;
     for (uint32_t b = gwarp(); b < NB; b += gwarps()) {
         uint32_t my_nb = NBR_NONE;
-        unsigned long long my_f = 0ull;
-        if (lane < ND) { my_nb = st.adj[(size_t)b * ND + lane]; my_f = st.fetch[(size_t)b * ND + lane]; }
+        if (lane < ND) my_nb = st.adj[(size_t)b * ND + lane];
         double a0 = st.Qn[(size_t)b * 64 + lane], a1 = st.Qn[(size_t)b * 64 + 32 + lane];
-        const unsigned any = __ballot_sync(0xffffffffu, my_f != 0ull);
+        const unsigned f0 = st.fetch[(size_t)b * 64 + lane], f1 = st.fetch[(size_t)b * 64 + 32 + lane];
+        unsigned any = f0 | f1;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) any |= __shfl_xor_sync(0xffffffffu, any, o);
         if (any) {
 #pragma unroll
             for (int d = 0; d < ND; ++d) {
                 if (!((any >> d) & 1u)) continue;
                 const uint32_t nb = __shfl_sync(0xffffffffu, my_nb, d);
-                const unsigned long long f = __shfl_sync(0xffffffffu, my_f, d);
                 const int j = d >> 1;
                 const double* src = st.phi + ((size_t)nb * ND + (d ^ 1)) * 32;
-                if ((f >> lane) & 1ull) { const double v = src[G::fidx(j, (int)lane)]; a0 += (d & 1) ? -v : v; }
-                if ((f >> (lane + 32)) & 1ull) { const double v = src[G::fidx(j, (int)lane + 32)]; a1 += (d & 1) ? -v : v; }
+                if ((f0 >> d) & 1u) { const double v = src[G::fidx(j, (int)lane)]; a0 += (d & 1) ? -v : v; }
+                if ((f1 >> d) & 1u) { const double v = src[G::fidx(j, (int)lane + 32)]; a1 += (d & 1) ? -v : v; }
             }
             st.Qn[(size_t)b * 64 + lane] = a0;
             st.Qn[(size_t)b * 64 + 32 + lane] = a1;

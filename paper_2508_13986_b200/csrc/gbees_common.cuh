@@ -70,7 +70,7 @@ struct Store {
     uint64_t* mask;      // [capB] active-cell bits (bit = local index)
     uint64_t* grown;     // [capB] cells whose Targets(c) have been inserted (autonomous f: grow once)
     uint64_t* keep;      // [capB] prune marks
-    uint64_t* fetch;     // [capB][2n] cells that must fetch an external inflow flux in pass 2
+    uint16_t* fetch;     // [capB][64] per cell: bit d = fetch the flux of external face d from the neighbour brick in pass 2
     uint32_t* adj;       // [capB][2n] neighbour brick rows: d = 2j (-e^j), 2j+1 (+e^j); NBR_NONE if absent
     uint32_t* slot_of;   // [capB] hashtable slot of a brick created by this step's grow
     ulonglong2* table;   // [slots] {brick key, row}
