@@ -83,148 +83,207 @@ __device__ __forceinline__ void decode_target(int t, int& j, int& sj, int& l, in
 //   activated (bit set in its brick's mask; the brick is created if absent).
 // GROW = false (Alg. 3 line "mark"): sources = all cells with P >= p*; the source and
 //   every existing target get a keep mark.
-// Block-cooperative: the sources of WPB bricks are compacted into shared memory, then the
-// (source, target) pairs are spread over all threads.
+// Bit-parallel per brick: one warp turns the sources' outflow flags into 2n slot masks O_d, then
+// every lane takes target classes t (a face step or a pair of steps), ANDs the masks of the steps
+// involved, shifts the result to the target slots and splits it by destination brick (own, face
+// neighbour, diagonal). Masks bound for the own brick and the 2n face neighbours are merged in
+// shared memory, so a brick costs O(2n + diagonals) global atomics instead of O(cells x targets).
+template <int NDIM>
+__device__ __forceinline__ unsigned long long edge_mask(int j, int side) {   // slots whose step (j, side) leaves the brick
+    unsigned long long e = 0ull;
+    const int SH = Geo<NDIM>::SH(j), MK = Geo<NDIM>::MK(j);
+    for (int l = 0; l < 64; ++l)
+        if (((l >> SH) & MK) == (side ? MK : 0)) e |= 1ull << l;
+    return e;
+}
+
+// GROW: activate the cells `bits` of the brick in row `row` (NBR_NONE: unknown, look `key` up and
+// create it if absent). Returns the bits this thread switched on; `key` then holds the brick's key.
+__device__ __forceinline__ unsigned long long grow_apply(const Params& p, const Store& st, DevState* ds, uint32_t NB0,
+                                                         uint64_t slots, int nd, uint32_t row, uint64_t key,
+                                                         unsigned long long bits) {
+    if (row == NBR_NONE) {
+        bool inserted;
+        const uint64_t s = ht_upsert(st.table, slots, key, inserted);
+        if (s == ~0ull) { atomicOr(&ds->err, E_TABLE_FULL); return 0ull; }
+        if (inserted) {
+            const uint32_t nr = atomicAdd(&ds->NB, 1u);
+            if (nr >= p.capB) { atomicOr(&ds->err, E_CAPACITY); return 0ull; }
+            st.bkey[nr] = key; st.slot_of[nr] = (uint32_t)s; st.grown[nr] = 0ull; st.mask[nr] = 0ull;
+            for (int d = 0; d < nd; ++d) st.adj[(size_t)nr * nd + d] = NBR_NONE;
+            __threadfence();
+            *reinterpret_cast<volatile unsigned long long*>(&st.table[s].y) = nr;
+        } else {
+            const uint32_t er = (uint32_t)*reinterpret_cast<volatile unsigned long long*>(&st.table[s].y);
+            if (er != NBR_NONE && er < NB0) row = er;       // existed before this launch (diagonal without adjacency)
+        }
+        // a brick created during this launch collects its bits in pend[slot] (folded in by link)
+        if (row == NBR_NONE) return bits & ~atomicOr((unsigned long long*)&st.pend[s], bits);
+    }
+    const unsigned long long want = bits & ~*reinterpret_cast<volatile unsigned long long*>(&st.mask[row]);
+    if (!want) return 0ull;
+    return want & ~atomicOr((unsigned long long*)&st.mask[row], want);
+}
+
 template <int NDIM, int DYN, bool GROW>
 __device__ void phase_targets(const Params& p, const Store& st, DevState* ds) {
     using G = Geo<NDIM>;
-    constexpr int NT = 2 * NDIM + 2 * NDIM * (NDIM - 1);
-    constexpr int ND = 2 * NDIM;
-    __shared__ uint32_t s_row[WPB * 64];
-    __shared__ uint32_t s_flag[WPB * 64];   // [0,2n): outflow bits (2j: lower, 2j+1: upper); [16,16+2n): at range border; [28,32)+: unused
-    __shared__ uint8_t s_loc[WPB * 64];
-    __shared__ unsigned s_cnt;
+    constexpr int ND = 2 * NDIM, NT = ND + 2 * NDIM * (NDIM - 1), OWN = ND;
+    __shared__ unsigned long long sO[WPB][ND];        // O_d: sources with outflow through face d
+    __shared__ unsigned long long sT[WPB][ND + 1];    // target bits per destination (face neighbours, own)
+    __shared__ uint32_t sAdj[WPB][ND];
+    __shared__ unsigned long long sEdge[ND];
+    __shared__ unsigned long long sQk[GROW ? WPB : 1][GROW ? NT : 1], sQm[GROW ? WPB : 1][GROW ? NT : 1];   // new cells: (brick key, bits)
+    __shared__ unsigned sQn[WPB];
+    if (threadIdx.x < ND) sEdge[threadIdx.x] = edge_mask<NDIM>(threadIdx.x >> 1, threadIdx.x & 1);
+    __syncthreads();
     const uint32_t NB0 = GROW ? ds->NB_before_grow : min(ds->NB, p.capB);
     const double scale = ds->scale;
     const uint64_t slots = ds->slots;
     const int32_t lo = (int32_t)(-p.bias), hi = (int32_t)(p.bias - 1);
-    const unsigned warp = threadIdx.x >> 5, lane = lane_id();
+    const unsigned w = threadIdx.x >> 5, lane = lane_id();
     unsigned long long n_new = 0;
     double smax = 0.0;
-    for (uint32_t base = blockIdx.x * WPB; base < NB0; base += gridDim.x * WPB) {   // block-uniform
-        if (threadIdx.x == 0) s_cnt = 0;
-        __syncthreads();
-        const uint32_t b = base + warp;
-        if (b < NB0) {
-            const uint64_t m = st.mask[b];
-            const uint64_t g = GROW ? st.grown[b] : 0ull;
-            const uint64_t cand = m & ~g;
-            if (cand) {                                                            // warp-uniform
-                const uint64_t bk = st.bkey[b];
-                int32_t B[NDIM];
-                unpack<NDIM>(p, bk, B);
-                uint64_t src = 0;
+    // new cells (GROW) are queued per warp as (brick key, bits) and expanded by all lanes below
+    auto account = [&](uint64_t key, unsigned long long fresh) {
+        if (!fresh) return;
+        const unsigned k = atomicAdd(&sQn[GROW ? w : 0], 1u);
+        sQk[GROW ? w : 0][GROW ? k : 0] = key;
+        sQm[GROW ? w : 0][GROW ? k : 0] = fresh;
+    };
+    for (uint32_t b = gwarp(); b < NB0; b += gwarps()) {   // warp-uniform
+        const uint64_t m = st.mask[b];
+        const uint64_t g = GROW ? st.grown[b] : 0ull;
+        const uint64_t cand = m & ~g;
+        if (!cand) continue;
+        const uint64_t bk = st.bkey[b];
+        int32_t B[NDIM];
+        unpack<NDIM>(p, bk, B);
+        unsigned fl[2] = {0u, 0u};
+        uint64_t src = 0;
 #pragma unroll
-                for (int hh = 0; hh < 2; ++hh) {
-                    const int l = (int)lane + 32 * hh;
-                    bool is_src = false;
-                    if ((cand >> l) & 1ull) is_src = scale * st.Q[(size_t)b * 64 + l] >= p.thresh;
-                    if (is_src) {
-                        int32_t c[NDIM];
-                        cell_coords<NDIM>(B, l, c);
-                        double ul[NDIM], uu[NDIM];
-                        face_velocities<NDIM, DYN>(p, c, ul, uu);
-                        uint32_t f = 0;
+        for (int hh = 0; hh < 2; ++hh) {
+            const int l = (int)lane + 32 * hh;
+            bool is_src = false;
+            if ((cand >> l) & 1ull) is_src = scale * st.Q[(size_t)b * 64 + l] >= p.thresh;
+            if (is_src) {
+                int32_t c[NDIM];
+                cell_coords<NDIM>(B, l, c);
+                double ul[NDIM], uu[NDIM];
+                face_velocities<NDIM, DYN>(p, c, ul, uu);
+                unsigned f = 0, border = 0;
 #pragma unroll
-                        for (int j = 0; j < NDIM; ++j) {
-                            f |= (ul[j] < 0.0 ? 1u : 0u) << (2 * j);
-                            f |= (uu[j] > 0.0 ? 1u : 0u) << (2 * j + 1);
-                            f |= (c[j] <= lo ? 1u : 0u) << (16 + 2 * j);
-                            f |= (c[j] >= hi ? 1u : 0u) << (16 + 2 * j + 1);
-                        }
-                        const unsigned k = atomicAdd(&s_cnt, 1u);
-                        s_row[k] = b; s_loc[k] = (uint8_t)l; s_flag[k] = f;
-                    }
-                    src |= (uint64_t)__ballot_sync(0xffffffffu, is_src) << (32 * hh);
+                for (int j = 0; j < NDIM; ++j) {
+                    f |= (ul[j] < 0.0 ? 1u : 0u) << (2 * j);
+                    f |= (uu[j] > 0.0 ? 1u : 0u) << (2 * j + 1);
+                    border |= (c[j] <= lo ? 1u : 0u) << (2 * j);
+                    border |= (c[j] >= hi ? 1u : 0u) << (2 * j + 1);
                 }
-                if (lane == 0 && src) {
-                    if (GROW) st.grown[b] = g | src;          // autonomous f: grow once
-                    else atomicOr((unsigned long long*)&st.keep[b], (unsigned long long)src);
+                if (f & border) {                        // a target would leave the packable range (A18)
+                    if (GROW) atomicOr(&ds->err, E_KEY_RANGE);
+                    f &= ~border;
                 }
+                fl[hh] = f;
             }
+            src |= (uint64_t)__ballot_sync(0xffffffffu, is_src) << (32 * hh);
         }
-        __syncthreads();
-        const unsigned total = s_cnt * NT;
-        for (unsigned w = threadIdx.x; w < total; w += blockDim.x) {
-            const unsigned src = w / NT;
-            const int t = (int)(w - src * NT);
+        if (!src) continue;
+        if (lane < ND) sAdj[w][lane] = st.adj[(size_t)b * ND + lane];
+        if (lane <= ND) sT[w][lane] = (!GROW && lane == OWN) ? src : 0ull;   // mark: sources keep themselves
+        if (lane == 0) sQn[w] = 0u;
+#pragma unroll
+        for (int d = 0; d < ND; ++d) {
+            const unsigned long long od = (unsigned long long)__ballot_sync(0xffffffffu, (fl[0] >> d) & 1u) |
+                                          ((unsigned long long)__ballot_sync(0xffffffffu, (fl[1] >> d) & 1u) << 32);
+            if (lane == 0) sO[w][d] = od;
+        }
+        if (GROW && lane == 0) st.grown[b] = g | src;            // autonomous f: grow once
+        __syncwarp();
+        for (int t = (int)lane; t < NT; t += 32) {
             int j, sj, l2, sl;
             decode_target<NDIM>(t, j, sj, l2, sl);
-            const uint32_t f = s_flag[src];
-            if (!((f >> (2 * j + sj)) & 1u)) continue;
-            if (l2 >= 0 && !((f >> (2 * l2 + sl)) & 1u)) continue;
-            bool bad = (f >> (16 + 2 * j + sj)) & 1u;
-            if (l2 >= 0) bad = bad || ((f >> (16 + 2 * l2 + sl)) & 1u);
-            if (bad) { if (GROW) atomicOr(&ds->err, E_KEY_RANGE); continue; }
-            const uint32_t r = s_row[src];
-            int tl = s_loc[src];
-            const uint64_t bk = st.bkey[r];
-            uint64_t tk = bk;
-            int carries = 0, cdir = 0;
-            {   // step along j
-                const int K = G::K(j), SH = G::SH(j), MK = (1 << K) - 1;
-                const int fld = (tl >> SH) & MK, nf = fld + (sj ? 1 : -1);
-                tl = (tl & ~(MK << SH)) | ((nf & MK) << SH);
-                if (nf < 0 || nf > MK) {
-                    const uint64_t unit = 1ull << ((NDIM - 1 - j) * p.bits);
-                    tk = sj ? tk + unit : tk - unit;
-                    ++carries; cdir = 2 * j + sj;
-                }
-            }
-            if (l2 >= 0) {   // step along l2
-                const int K = G::K(l2), SH = G::SH(l2), MK = (1 << K) - 1;
-                const int fld = (tl >> SH) & MK, nf = fld + (sl ? 1 : -1);
-                tl = (tl & ~(MK << SH)) | ((nf & MK) << SH);
-                if (nf < 0 || nf > MK) {
-                    const uint64_t unit = 1ull << ((NDIM - 1 - l2) * p.bits);
-                    tk = sl ? tk + unit : tk - unit;
-                    ++carries; cdir = 2 * l2 + sl;
-                }
-            }
-            const unsigned long long bit = 1ull << tl;
-            uint32_t row = NBR_NONE;
-            if (carries == 0) row = r;
-            else if (carries == 1) row = st.adj[(size_t)r * ND + cdir];
-            if (!GROW) {
-                if (row == NBR_NONE) row = ht_find(st.table, slots, tk);
-                if (row != NBR_NONE) atomicOr((unsigned long long*)&st.keep[row], bit);
+            const int d1 = 2 * j + sj;
+            unsigned long long S = sO[w][d1];
+            if (l2 >= 0) S &= sO[w][2 * l2 + sl];
+            if (!S) continue;
+            const int s1 = 1 << G::SH(j), w1 = G::MK(j) * s1;
+            unsigned long long in = S & ~sEdge[d1], cr = S & sEdge[d1];     // stay in the brick / cross face d1
+            in = sj ? in << s1 : in >> s1;
+            cr = sj ? cr >> w1 : cr << w1;
+            if (l2 < 0) {
+                if (in) atomicOr(&sT[w][OWN], in);
+                if (cr) atomicOr(&sT[w][d1], cr);
                 continue;
             }
-            // GROW. A brick that existed before this launch (row < NB0) takes the bit in its mask;
-            // a brick created during this launch collects bits in pend[slot] (folded in by link).
-            bool fresh;   // did THIS thread activate the cell?
-            if (row != NBR_NONE && row < NB0) {
-                fresh = !(atomicOr((unsigned long long*)&st.mask[row], bit) & bit);
-            } else {
-                bool inserted;
-                const uint64_t s = ht_upsert(st.table, slots, tk, inserted);
-                if (s == ~0ull) { atomicOr(&ds->err, E_TABLE_FULL); continue; }
-                if (inserted) {
-                    const uint32_t nr = atomicAdd(&ds->NB, 1u);
-                    if (nr >= p.capB) { atomicOr(&ds->err, E_CAPACITY); continue; }
-                    st.bkey[nr] = tk; st.slot_of[nr] = (uint32_t)s; st.grown[nr] = 0ull; st.mask[nr] = 0ull;
-#pragma unroll
-                    for (int d = 0; d < ND; ++d) st.adj[(size_t)nr * ND + d] = NBR_NONE;
-                    __threadfence();
-                    *reinterpret_cast<volatile unsigned long long*>(&st.table[s].y) = nr;
-                    fresh = !(atomicOr((unsigned long long*)&st.pend[s], bit) & bit);
+            const int d2 = 2 * l2 + sl;
+            const int s2 = 1 << G::SH(l2), w2 = G::MK(l2) * s2;
+            const unsigned long long e2 = sEdge[d2];
+            unsigned long long p00 = in & ~e2, p01 = in & e2, p10 = cr & ~e2, p11 = cr & e2;
+            p00 = sl ? p00 << s2 : p00 >> s2;
+            p10 = sl ? p10 << s2 : p10 >> s2;
+            p01 = sl ? p01 >> w2 : p01 << w2;
+            p11 = sl ? p11 >> w2 : p11 << w2;
+            if (p00) atomicOr(&sT[w][OWN], p00);
+            if (p01) atomicOr(&sT[w][d2], p01);
+            if (p10) atomicOr(&sT[w][d1], p10);
+            if (p11) {   // diagonal brick: through the adjacency of either face neighbour, else by key
+                uint32_t row = NBR_NONE;
+                const uint32_t r1 = sAdj[w][d1], r2 = sAdj[w][d2];
+                if (r1 != NBR_NONE) row = st.adj[(size_t)r1 * ND + d2];
+                if (row == NBR_NONE && r2 != NBR_NONE) row = st.adj[(size_t)r2 * ND + d1];
+                const uint64_t u1 = 1ull << ((NDIM - 1 - j) * p.bits), u2 = 1ull << ((NDIM - 1 - l2) * p.bits);
+                uint64_t key = sj ? bk + u1 : bk - u1;
+                key = sl ? key + u2 : key - u2;
+                if (GROW) {
+                    account(key, grow_apply(p, st, ds, NB0, slots, ND, row, key, p11));
                 } else {
-                    const uint32_t er = (uint32_t)*reinterpret_cast<volatile unsigned long long*>(&st.table[s].y);
-                    if (er != NBR_NONE && er < NB0) fresh = !(atomicOr((unsigned long long*)&st.mask[er], bit) & bit);
-                    else fresh = !(atomicOr((unsigned long long*)&st.pend[s], bit) & bit);
+                    if (row == NBR_NONE) row = ht_find(st.table, slots, key);
+                    if (row != NBR_NONE) {
+                        const unsigned long long x = p11 & st.mask[row];
+                        if (x) atomicOr((unsigned long long*)&st.keep[row], x);
+                    }
                 }
             }
-            if (fresh) {   // new cell: count it, fold its CFL term into the running maximum (Eq. 8)
-                ++n_new;
-                int32_t TB[NDIM], tc[NDIM];
-                unpack<NDIM>(p, tk, TB);
-                cell_coords<NDIM>(TB, tl, tc);
-                double ul[NDIM], uu[NDIM];
-                face_velocities<NDIM, DYN>(p, tc, ul, uu);
-                smax = fmax(smax, cfl_term<NDIM>(p, ul));
+        }
+        __syncwarp();
+        if (lane <= ND) {   // one lane per destination: own brick and the 2n face neighbours
+            const unsigned long long T = sT[w][lane];
+            if (T) {
+                const uint32_t row = lane == OWN ? b : sAdj[w][lane];
+                if (GROW) {
+                    uint64_t key = bk;
+                    if (lane != OWN) {
+                        const uint64_t u1 = 1ull << ((NDIM - 1 - (int)(lane >> 1)) * p.bits);
+                        key = (lane & 1) ? bk + u1 : bk - u1;
+                    }
+                    account(key, grow_apply(p, st, ds, NB0, slots, ND, row, key, T));
+                } else if (row != NBR_NONE) {
+                    const unsigned long long x = T & st.mask[row];
+                    if (x) atomicOr((unsigned long long*)&st.keep[row], x);
+                }
             }
         }
-        __syncthreads();
+        __syncwarp();
+        if (GROW) {   // count the new cells and fold their CFL terms into the running maximum (Eq. 8)
+            const unsigned nq = sQn[w];
+            for (unsigned k = 0; k < nq; ++k) {
+                const unsigned long long fresh = sQm[w][k];
+                int32_t TB[NDIM];
+                unpack<NDIM>(p, sQk[w][k], TB);
+#pragma unroll
+                for (int hh = 0; hh < 2; ++hh) {
+                    const int tl = (int)lane + 32 * hh;
+                    if (!((fresh >> tl) & 1ull)) continue;
+                    int32_t tc[NDIM];
+                    cell_coords<NDIM>(TB, tl, tc);
+                    double ul[NDIM], uu[NDIM];
+                    face_velocities<NDIM, DYN>(p, tc, ul, uu);
+                    smax = fmax(smax, cfl_term<NDIM>(p, ul));
+                    ++n_new;
+                }
+            }
+            __syncwarp();
+        }
     }
     if (GROW) {
         const double nn = block_sum((double)n_new);     // exact: counts << 2^53
