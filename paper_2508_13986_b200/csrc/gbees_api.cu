@@ -16,35 +16,69 @@ using namespace gbees;
 // ------------------------------------------------------------------------------------------------
 // __global__ wrappers (one per phase; Params / Store by value in the constant bank)
 // ------------------------------------------------------------------------------------------------
-#define GP const __grid_constant__ Params p, const __grid_constant__ Store st, DevState* ds
-__global__ void k_begin(DevState* ds, double dt_cap) {
-    ds->N_before_grow = ds->N;
-    ds->NB_before_grow = ds->NB;
+#define GP const __grid_constant__ Params p, const __grid_constant__ Store st_in, DevState* ds
+#define ST const Store st = resolve(st_in, ds)
+// guard: 0 = always run, 1 = part of a step (runs if ds->go), 2 = part of a prune (runs if ds->prune_ok)
+#define GUARD(g) if (((g) == 1 && !ds->go) || ((g) == 2 && !ds->prune_ok)) return
+
+// start of gbees_step: one step with the caller's cap
+__global__ void k_begin_step(DevState* ds, double dt_cap) {
+    ds->t_target = 1e300;
+    ds->step_limit = ds->steps + 1ull;
+    begin_step(ds);
     ds->dt_cap = dt_cap;
 }
+// start of gbees_run: the device decides step by step whether to go on
+__global__ void k_begin_run(DevState* ds, double t_target, unsigned long long step_limit) {
+    ds->t_target = t_target;
+    ds->step_limit = step_limit;
+    ds->prune_ok = 0;
+    begin_step(ds);
+}
+__global__ void k_set_prune_ok(DevState* ds) { ds->prune_ok = 1; }
 template <int NDIM, int DYN>
-__global__ void __launch_bounds__(TPB) k_grow(GP) { phase_targets<NDIM, DYN, true>(p, st, ds); }
+__global__ void __launch_bounds__(TPB) k_grow(GP) { GUARD(1); ST; phase_targets<NDIM, DYN, true>(p, st, ds); }
 template <int NDIM, int DYN>
-__global__ void __launch_bounds__(TPB) k_mark(GP) { phase_targets<NDIM, DYN, false>(p, st, ds); }
+__global__ void __launch_bounds__(TPB) k_mark(GP) { GUARD(2); ST; phase_targets<NDIM, DYN, false>(p, st, ds); }
 template <int NDIM, bool ALL>
-__global__ void __launch_bounds__(TPB) k_link(GP) { phase_link<NDIM, ALL>(p, st, ds); }
-template <int NDIM, int DYN>
-__global__ void __launch_bounds__(TPB) k_flux1(GP) { phase_flux1<NDIM, DYN>(p, st, ds); }
+__global__ void __launch_bounds__(TPB) k_link(GP, int guard) { GUARD(guard); ST; phase_link<NDIM, ALL>(p, st, ds); }
+template <int NDIM, int DYN, bool FAST>
+__global__ void __launch_bounds__(TPB) k_flux1(GP) { GUARD(1); ST; phase_flux1<NDIM, DYN, FAST>(p, st, ds); }
+// pass 2 + finish; a step that does not execute also cancels the prune enqueued behind it
 template <int NDIM>
-__global__ void __launch_bounds__(TPB) k_flux2(GP) { phase_flux2<NDIM>(p, st, ds); }
+__global__ void __launch_bounds__(TPB) k_flux2(GP) {
+    if (!ds->go) { if (gtid() == 0) ds->prune_ok = 0; return; }
+    ST;
+    phase_flux2_finish<NDIM>(p, st, ds);
+}
 template <int NDIM, int DYN>
-__global__ void __launch_bounds__(TPB) k_smax(GP) { phase_smax<NDIM, DYN>(p, st, ds); }
-__global__ void __launch_bounds__(TPB) k_sum(GP, int count) { phase_sum(p, st, ds, count != 0); }
-// mode: 0 = after a step, 1 = renormalise only (init / correct / prune), 2 = sum only (import)
-__global__ void __launch_bounds__(TPB) k_finish(GP, unsigned nparts, int mode) {
+__global__ void __launch_bounds__(TPB) k_smax(GP, int guard) { GUARD(guard); ST; phase_smax<NDIM, DYN>(p, st, ds); }
+__global__ void __launch_bounds__(TPB) k_sum(GP, int count, int guard) { GUARD(guard); ST; phase_sum(p, st, ds, count != 0); }
+// mode: 1 = renormalise (init / correct / prune), 2 = sum only (import)
+__global__ void __launch_bounds__(TPB) k_finish(GP, unsigned nparts, int mode, int guard) {
+    GUARD(guard);
+    ST;
     Params q = p;
     if (mode == 2) q.normalise = 0;
-    finish_sum(q, st, ds, nparts, mode == 0);
+    finish_sum(q, st, ds, nparts, false);
+    if (guard == 2 && threadIdx.x == 0) begin_step(ds);   // the prune changed N / NB: refresh the next step's setup
 }
-__global__ void __launch_bounds__(TPB) k_prune_scan(GP) { phase_prune_scan(p, st, ds); }
-__global__ void __launch_bounds__(TPB) k_prune_move(GP) { phase_prune_move(p, st, ds); }
-__global__ void __launch_bounds__(TPB) k_zero_tail(GP) { phase_zero_tail(p, st, ds); }
+// prune prologue: clear the marks and the scan descriptors (sizes are only known on the device)
+__global__ void __launch_bounds__(TPB) k_prune_prep(GP) {
+    GUARD(2);
+    ST;
+    const uint32_t NB = min(ds->NB, p.capB);
+    for (uint32_t i = gtid(); i < NB; i += gthreads()) st.keep[i] = 0ull;
+    const uint32_t ntiles = (NB + SCAN_TILE - 1) / SCAN_TILE + 1;
+    for (uint32_t i = gtid(); i < ntiles; i += gthreads()) st.tile_state[i] = 0ull;
+    if (gtid() == 0) ds->tile_counter = 0u;
+}
+__global__ void __launch_bounds__(TPB) k_prune_scan(GP) { GUARD(2); ST; phase_prune_scan(p, st, ds); }
+__global__ void __launch_bounds__(TPB) k_prune_move(GP) { GUARD(2); ST; phase_prune_move(p, st, ds); }
+__global__ void __launch_bounds__(TPB) k_zero_tail(GP) { GUARD(2); ST; phase_zero_tail(p, st, ds); }
+// after the move: survivors live in Qn and in the second metadata buffers -> flip both parities
 __global__ void k_after_compact(const __grid_constant__ Params p, DevState* ds) {
+    GUARD(2);
     ds->prune_scanned += ds->N;
     ds->prunes += 1;
     ds->NB = ds->NB_after_prune;
@@ -53,26 +87,27 @@ __global__ void k_after_compact(const __grid_constant__ Params p, DevState* ds) 
     ds->smax_bits = 0ull;
     ds->N = 0ull;                      // recounted by k_sum
     ds->tile_counter = 0u;
+    ds->parity ^= 3u;
 }
 // resize the active table for the current brick count; recount = also reset N and the CFL maximum
 __global__ void k_set_slots(const __grid_constant__ Params p, DevState* ds, int recount) {
     ds->slots = table_slots_for(p, min(ds->NB, p.capB));
     if (recount) { ds->smax_bits = 0ull; ds->N = 0ull; }
 }
-__global__ void __launch_bounds__(TPB) k_clear_table(const __grid_constant__ Store st, const DevState* ds) {
-    phase_clear_table(st, ds);
-}
-__global__ void __launch_bounds__(TPB) k_rebuild(GP) { phase_rebuild(p, st, ds); }
+__global__ void __launch_bounds__(TPB) k_clear_table(GP, int guard) { GUARD(guard); ST; phase_clear_table(st, ds); }
+__global__ void __launch_bounds__(TPB) k_rebuild(GP, int guard) { GUARD(guard); ST; phase_rebuild(p, st, ds); }
 template <int NDIM, bool FILL>
 __global__ void __launch_bounds__(TPB) k_init_gaussian(GP, const __grid_constant__ GaussArgs g) {
+    ST;
     phase_init_gaussian<NDIM, FILL>(p, st, ds, g);
 }
 template <int NDIM>
-__global__ void __launch_bounds__(TPB) k_correct(GP, const __grid_constant__ GaussArgs g) { phase_correct<NDIM>(p, st, ds, g); }
+__global__ void __launch_bounds__(TPB) k_correct(GP, const __grid_constant__ GaussArgs g) { ST; phase_correct<NDIM>(p, st, ds, g); }
 template <int NDIM>
-__global__ void __launch_bounds__(TPB) k_export(GP, int32_t* keys, double* out) { phase_export<NDIM>(p, st, ds, keys, out); }
+__global__ void __launch_bounds__(TPB) k_export(GP, int32_t* keys, double* out) { ST; phase_export<NDIM>(p, st, ds, keys, out); }
 template <int NDIM, bool FILL>
 __global__ void __launch_bounds__(TPB) k_import(GP, const int32_t* keys, const double* vals, uint64_t count) {
+    ST;
     phase_import<NDIM, FILL>(p, st, ds, keys, vals, count);
 }
 
@@ -232,21 +267,21 @@ int sync_state(gbees_ctx* c) {
 int rebuild_all(gbees_ctx* c, int finish_mode) {
     phase(c, GBEES_PH_REBUILD, 3, [&] {
         k_set_slots<<<1, 1, 0, c->stream>>>(c->p, c->d_st, 1);
-        k_clear_table<<<c->grid, TPB, 0, c->stream>>>(c->st, c->d_st);
-        k_rebuild<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
+        k_clear_table<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 0);
+        k_rebuild<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 0);
     });
     int rc = GBEES_OK;
     phase(c, GBEES_PH_RELINK, 2, [&] {
         rc = dispatch(c, [&](auto N_, auto D_) {
-            k_link<decltype(N_)::value, true><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
-            k_smax<decltype(N_)::value, decltype(D_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
+            k_link<decltype(N_)::value, true><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 0);
+            k_smax<decltype(N_)::value, decltype(D_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 0);
             return GBEES_OK;
         });
     });
     if (rc) return fail(c, rc, "unsupported (n, dynamics) pair");
     phase(c, GBEES_PH_SUM, 2, [&] {
-        k_sum<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 1);
-        k_finish<<<1, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, c->grid, finish_mode);
+        k_sum<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 1, 0);
+        k_finish<<<1, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, c->grid, finish_mode, 0);
     });
     CU(cudaGetLastError());
     return GBEES_OK;
@@ -266,7 +301,7 @@ int reset_grid(gbees_ctx* c) {
     z.slots = c->p.slots;
     *c->h_st = z;
     CU(cudaMemcpyAsync(c->d_st, c->h_st, sizeof(DevState), cudaMemcpyHostToDevice, c->stream));
-    k_clear_table<<<c->grid, TPB, 0, c->stream>>>(c->st, c->d_st);
+    k_clear_table<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 0);
     c->launches += 1;
     c->n_inserted = c->n_pruned = 0;
     return GBEES_OK;
@@ -451,48 +486,90 @@ int gbees_import(gbees_ctx* c, const double* origin, const int32_t* keys, const 
     return sync_state(c);
 }
 
+// enqueue the launches of one step (each runs only if the device's go flag is set)
+static int enqueue_step(gbees_ctx* c) {
+    int rc = dispatch(c, [&](auto N_, auto D_) {
+        constexpr int NN = decltype(N_)::value, DD = decltype(D_)::value;
+        if (!c->no_grow) {
+            phase(c, GBEES_PH_GROW, 1, [&] { k_grow<NN, DD><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st); });
+            phase(c, GBEES_PH_LINK, 1, [&] { k_link<NN, false><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 1); });
+        }
+        phase(c, GBEES_PH_PASSA, 1, [&] {
+            constexpr size_t smem = sizeof(Flux1Smem<NN>) * WPB;
+            static bool attr_set = false;
+            if (!attr_set) {
+                cudaFuncSetAttribute(k_flux1<NN, DD, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+                cudaFuncSetAttribute(k_flux1<NN, DD, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+                attr_set = true;
+            }
+            if (c->p.hi_res && !c->p.limiter) k_flux1<NN, DD, true><<<c->grid, TPB, smem, c->stream>>>(c->p, c->st, c->d_st);
+            else k_flux1<NN, DD, false><<<c->grid, TPB, smem, c->stream>>>(c->p, c->st, c->d_st);
+        });
+        phase(c, GBEES_PH_PASSB, 1, [&] { k_flux2<NN><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st); });
+        return GBEES_OK;
+    });
+    if (rc) return fail(c, rc, "unsupported (n, dynamics) pair");
+    return GBEES_OK;
+}
+
+// enqueue the launches of one prune (each runs only if the device's prune_ok flag is set)
+static int enqueue_prune(gbees_ctx* c) {
+    int rc = GBEES_OK;
+    phase(c, GBEES_PH_MARK, 2, [&] {
+        k_prune_prep<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
+        rc = dispatch(c, [&](auto N_, auto D_) {
+            k_mark<decltype(N_)::value, decltype(D_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
+            return GBEES_OK;
+        });
+    });
+    if (rc) return fail(c, rc, "unsupported (n, dynamics) pair");
+    phase(c, GBEES_PH_COMPACT, 4, [&] {
+        k_prune_scan<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
+        k_prune_move<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
+        k_zero_tail<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
+        k_after_compact<<<1, 1, 0, c->stream>>>(c->p, c->d_st);
+    });
+    phase(c, GBEES_PH_REBUILD, 2, [&] {
+        k_clear_table<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 2);
+        k_rebuild<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 2);
+    });
+    phase(c, GBEES_PH_RELINK, 4, [&] {
+        rc = dispatch(c, [&](auto N_, auto D_) {
+            k_link<decltype(N_)::value, true><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 2);
+            k_smax<decltype(N_)::value, decltype(D_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 2);
+            return GBEES_OK;
+        });
+        k_sum<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 1, 2);
+        k_finish<<<1, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, c->grid, 1, 2);
+    });
+    return GBEES_OK;
+}
+
+// the grid outgrew the active table: rehash into a larger one (adjacency is unaffected)
+static int rehash_if_needed(gbees_ctx* c) {
+    if (!((double)c->h_st->NB > c->p.load_factor * (double)c->h_st->slots && c->h_st->slots < c->p.slots)) return GBEES_OK;
+    phase(c, GBEES_PH_REBUILD, 3, [&] {
+        k_set_slots<<<1, 1, 0, c->stream>>>(c->p, c->d_st, 0);
+        k_clear_table<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 0);
+        k_rebuild<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 0);
+    });
+    return sync_state(c);
+}
+
 int gbees_step(gbees_ctx* c, double* dt) {
     if (!c || !dt) return GBEES_ERR_ARG;
     if (c->sticky) return c->sticky;
     CU(cudaSetDevice(c->device));
     if (c->h_st->N == 0) return fail(c, GBEES_ERR_DEGENERATE, "empty grid");
     const unsigned long long n_before = c->h_st->N;
-    int rc = dispatch(c, [&](auto N_, auto D_) {
-        constexpr int NN = decltype(N_)::value, DD = decltype(D_)::value;
-        phase(c, GBEES_PH_GROW, c->no_grow ? 1 : 2, [&] {
-            k_begin<<<1, 1, 0, c->stream>>>(c->d_st, *dt);
-            if (!c->no_grow) k_grow<NN, DD><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
-        });
-        if (!c->no_grow)
-            phase(c, GBEES_PH_LINK, 1, [&] { k_link<NN, false><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st); });
-        phase(c, GBEES_PH_PASSA, 1, [&] {
-            constexpr size_t smem = sizeof(Flux1Smem<NN>) * WPB;
-            static bool attr_set = false;
-            if (!attr_set) { cudaFuncSetAttribute(k_flux1<NN, DD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_set = true; }
-            k_flux1<NN, DD><<<c->grid, TPB, smem, c->stream>>>(c->p, c->st, c->d_st);
-        });
-        phase(c, GBEES_PH_PASSB, 2, [&] {
-            k_flux2<NN><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
-            k_finish<<<1, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, c->grid, 0);
-        });
-        return GBEES_OK;
-    });
-    if (rc) return fail(c, rc, "unsupported (n, dynamics) pair");
+    phase(c, GBEES_PH_GROW, 1, [&] { k_begin_step<<<1, 1, 0, c->stream>>>(c->d_st, *dt); });
+    int rc = enqueue_step(c);
+    if (rc) return rc;
     CU(cudaGetLastError());
-    std::swap(c->st.Q, c->st.Qn);          // pass 2 left the new masses in Qn
     if ((rc = sync_state(c))) return rc;
     c->n_inserted = (int64_t)c->h_st->N - (int64_t)n_before;
     *dt = c->h_st->dt;
-    if ((double)c->h_st->NB > c->p.load_factor * (double)c->h_st->slots && c->h_st->slots < c->p.slots) {
-        // the grid outgrew the active table: rehash into a larger one (adjacency is unaffected)
-        phase(c, GBEES_PH_REBUILD, 3, [&] {
-            k_set_slots<<<1, 1, 0, c->stream>>>(c->p, c->d_st, 0);
-            k_clear_table<<<c->grid, TPB, 0, c->stream>>>(c->st, c->d_st);
-            k_rebuild<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
-        });
-        if ((rc = sync_state(c))) return rc;
-    }
-    return GBEES_OK;
+    return rehash_if_needed(c);
 }
 
 int gbees_prune(gbees_ctx* c) {
@@ -500,42 +577,11 @@ int gbees_prune(gbees_ctx* c) {
     if (c->sticky) return c->sticky;
     CU(cudaSetDevice(c->device));
     const unsigned long long N = c->h_st->N;
-    const uint32_t NB = c->h_st->NB;
     if (N == 0) return fail(c, GBEES_ERR_DEGENERATE, "empty grid");
-    int rc = GBEES_OK;
-    phase(c, GBEES_PH_MARK, 2, [&] {
-        cudaMemsetAsync(c->st.keep, 0, (size_t)NB * 8, c->stream);
-        rc = dispatch(c, [&](auto N_, auto D_) {
-            k_mark<decltype(N_)::value, decltype(D_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
-            return GBEES_OK;
-        });
-    });
-    if (rc) return fail(c, rc, "unsupported (n, dynamics) pair");
-    phase(c, GBEES_PH_COMPACT, 6, [&] {
-        cudaMemsetAsync(c->st.tile_state, 0, (size_t)((NB + SCAN_TILE - 1) / SCAN_TILE + 1) * 8, c->stream);
-        cudaMemsetAsync(&c->d_st->tile_counter, 0, sizeof(unsigned), c->stream);
-        k_prune_scan<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
-        k_prune_move<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
-        k_zero_tail<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
-        k_after_compact<<<1, 1, 0, c->stream>>>(c->p, c->d_st);
-    });
-    std::swap(c->st.Q, c->st.Qn);
-    std::swap(c->st.bkey, c->st.bkey2);
-    std::swap(c->st.mask, c->st.mask2);
-    std::swap(c->st.grown, c->st.grown2);
-    phase(c, GBEES_PH_REBUILD, 2, [&] {
-        k_clear_table<<<c->grid, TPB, 0, c->stream>>>(c->st, c->d_st);
-        k_rebuild<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
-    });
-    phase(c, GBEES_PH_RELINK, 4, [&] {
-        rc = dispatch(c, [&](auto N_, auto D_) {
-            k_link<decltype(N_)::value, true><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
-            k_smax<decltype(N_)::value, decltype(D_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
-            return GBEES_OK;
-        });
-        k_sum<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 1);
-        k_finish<<<1, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, c->grid, 1);
-    });
+    k_set_prune_ok<<<1, 1, 0, c->stream>>>(c->d_st);
+    c->launches += 1;
+    int rc = enqueue_prune(c);
+    if (rc) return rc;
     CU(cudaGetLastError());
     if ((rc = sync_state(c))) return rc;
     c->n_pruned = (int64_t)N - (int64_t)c->h_st->N;
@@ -557,8 +603,8 @@ int gbees_correct(gbees_ctx* c, const double* z, const double* R) {
             k_correct<decltype(N_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, g);
             return GBEES_OK;
         });
-        k_sum<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 0);
-        k_finish<<<1, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, c->grid, 1);
+        k_sum<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 0, 0);
+        k_finish<<<1, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, c->grid, 1, 0);
     });
     CU(cudaGetLastError());
     return sync_state(c);
@@ -597,7 +643,7 @@ int gbees_export(gbees_ctx* c, int32_t* keys, double* pv, int64_t cap, int64_t* 
     return GBEES_OK;
 }
 
-// host loop over gbees_step / gbees_prune: the reference behaviour of gbees_run (opts.run_mode = 1)
+// host loop over gbees_step / gbees_prune with a host round trip per call (opts.run_mode = 1)
 static int run_host_loop(gbees_ctx* c, double t_target, int64_t max_steps, int prune_every, int64_t* steps_done) {
     int64_t k = 0;
     int rc = GBEES_OK;
@@ -611,11 +657,46 @@ static int run_host_loop(gbees_ctx* c, double t_target, int64_t max_steps, int p
     return rc;
 }
 
+// Step loop without host round trips (PAPER.md:170-172 keeps the whole loop on the device; here the
+// device decides per step whether the enqueued launches execute, and the host only reads the state
+// back once per chunk of steps).
 int gbees_run(gbees_ctx* c, double t_target, int64_t max_steps, int prune_every, int64_t* steps_done) {
     if (!c) return GBEES_ERR_ARG;
     if (c->sticky) return c->sticky;
     if (steps_done) *steps_done = 0;
-    return run_host_loop(c, t_target, max_steps, prune_every, steps_done);
+    if (c->run_mode == 1) return run_host_loop(c, t_target, max_steps, prune_every, steps_done);
+    CU(cudaSetDevice(c->device));
+    if (c->h_st->N == 0) return fail(c, GBEES_ERR_DEGENERATE, "empty grid");
+    if (max_steps <= 0 || !(c->h_st->t < t_target)) return GBEES_OK;
+    const unsigned long long steps0 = c->h_st->steps;
+    const unsigned long long limit = (unsigned long long)max_steps > (~0ull >> 1) - steps0 ? (~0ull >> 1) : steps0 + (unsigned long long)max_steps;
+    const unsigned long long n_before = c->h_st->N;
+    k_begin_run<<<1, 1, 0, c->stream>>>(c->d_st, t_target, limit);
+    c->launches += 1;
+    int rc = GBEES_OK;
+    int64_t k = 0;     // steps enqueued
+    for (;;) {
+        int64_t chunk = 16;
+        if (c->h_st->dt > 0.0 && t_target < 1e299) {     // do not enqueue far past the expected end
+            const double est = (t_target - c->h_st->t) / c->h_st->dt;
+            if (est < (double)chunk) chunk = (int64_t)est + 2;
+        }
+        if (chunk > max_steps - k) chunk = max_steps - k;
+        for (int64_t i = 0; i < chunk; ++i) {
+            if ((rc = enqueue_step(c))) return rc;
+            ++k;
+            if (prune_every > 0 && k % prune_every == 0 && (rc = enqueue_prune(c))) return rc;
+        }
+        CU(cudaGetLastError());
+        if ((rc = sync_state(c))) break;
+        if ((rc = rehash_if_needed(c))) break;
+        if (!c->h_st->go || k >= max_steps) break;
+    }
+    c->n_inserted = (int64_t)c->h_st->N - (int64_t)n_before;
+    if (steps_done) *steps_done = (int64_t)(c->h_st->steps - steps0);
+    if (rc) return rc;
+    if (c->h_st->N == 0) return fail(c, GBEES_ERR_DEGENERATE, "prune removed every cell");
+    return GBEES_OK;
 }
 
 int gbees_count(gbees_ctx* c, int64_t* count) {

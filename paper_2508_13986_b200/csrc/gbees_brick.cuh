@@ -371,7 +371,8 @@ struct Flux1Smem {
     uint8_t list[64];
 };
 
-template <int NDIM, int DYN>
+// FAST = true: production setting (hi_res on, MC limiter) compiled in; false: flags read at run time
+template <int NDIM, int DYN, bool FAST>
 __device__ void phase_flux1(const Params& p, const Store& st, DevState* ds) {
     using G = Geo<NDIM>;
     using SM = Flux1Smem<NDIM>;
@@ -381,7 +382,7 @@ __device__ void phase_flux1(const Params& p, const Store& st, DevState* ds) {
     SM& sm = reinterpret_cast<SM*>(smem_raw)[w];
     const uint32_t NB = min(ds->NB, p.capB);
     const double dt = step_dt(p, ds);
-    const bool hires = p.hi_res != 0, nolim = p.limiter != 0;
+    const bool hires = FAST || p.hi_res != 0, nolim = !FAST && p.limiter != 0;
     const double* __restrict__ Q = st.Q;
     double tau[NDIM];
 #pragma unroll
@@ -576,7 +577,17 @@ __device__ inline void phase_sum(const Params& p, const Store& st, DevState* ds,
     }
 }
 
-// one block: add the partials in index order, set the scale. after_step: advance t, count.
+// decide on the device whether the next enqueued step executes, and set it up (thread 0 of one block)
+__device__ __forceinline__ void begin_step(DevState* ds) {
+    const double t = ds->t, tt = ds->t_target;
+    ds->go = (t < tt) && (ds->steps < ds->step_limit) && ds->err == 0 && ds->N > 0ull;
+    ds->dt_cap = tt < 1e299 ? tt - t : 0.0;
+    ds->N_before_grow = ds->N;
+    ds->NB_before_grow = ds->NB;
+}
+
+// one block: add the partials in index order, set the scale. after_step: advance t, count, flip
+// the Q/Qn parity (pass 2 left the new masses in Qn) and set up the next step.
 __device__ inline void finish_sum(const Params& p, const Store& st, DevState* ds, unsigned nparts, bool after_step) {
     double v = 0.0;
     for (unsigned k = threadIdx.x; k < nparts; k += blockDim.x) v += st.partial[k];
@@ -598,7 +609,28 @@ __device__ inline void finish_sum(const Params& p, const Store& st, DevState* ds
             ds->steps += 1;
             ds->cell_updates += ds->N;
             ds->inserted_total += ds->N - ds->N_before_grow;
+            ds->parity ^= 1u;
+            ds->prune_ok = 1;
+            begin_step(ds);
         }
+    }
+}
+
+// pass 2 + mass sum + step bookkeeping in one launch: the last block to finish (ticket) adds the
+// per-block partials in index order (deterministic) and closes the step.
+template <int NDIM>
+__device__ void phase_flux2_finish(const Params& p, const Store& st, DevState* ds) {
+    __shared__ bool s_last;
+    phase_flux2<NDIM>(p, st, ds);
+    if (threadIdx.x == 0) {
+        __threadfence();
+        s_last = atomicAdd(&ds->ticket, 1u) == gridDim.x - 1;
+    }
+    __syncthreads();
+    if (s_last) {
+        __threadfence();
+        finish_sum(p, st, ds, gridDim.x, true);
+        if (threadIdx.x == 0) ds->ticket = 0;
     }
 }
 

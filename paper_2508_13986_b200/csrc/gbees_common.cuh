@@ -54,8 +54,12 @@ struct DevState {
     unsigned long long inserted_total;   // cells created by grow since init
     unsigned long long prune_scanned;    // sum over prunes of the cell count scanned
     unsigned long long prunes;
-    unsigned int parity;                 // persistent loop: bit 0 = Q/Qn swapped, bit 1 = metadata buffers swapped
+    unsigned int parity;                 // bit 0 = Q/Qn swapped, bit 1 = metadata double buffers swapped (resolve())
     unsigned int export_count;           // export: next output row
+    double t_target;                     // gbees_run: advance until t == t_target ...
+    unsigned long long step_limit;       // ... or until steps == step_limit
+    int go;                              // the step being enqueued executes (decided on the device by begin_step)
+    int prune_ok;                        // the last enqueued step executed: the prune that follows it runs
     unsigned long long phase_ns[12];     // persistent loop: device-timer ns per phase (index = GBEES_PH_*)
     unsigned long long slots;            // hashtable slots in use (<= Params::slots), resized at rehash
 };
@@ -82,6 +86,20 @@ struct Store {
     unsigned long long* tile_state;  // scan descriptors
     double* partial;     // block partial sums
 };
+
+// The host never swaps pointers: every kernel resolves the double buffers from the device parity
+// word, so whole runs can be enqueued without a host round trip per step.
+__device__ __forceinline__ Store resolve(const Store& in, const DevState* ds) {
+    Store s = in;
+    const unsigned par = ds->parity;
+    if (par & 1u) { double* t = s.Q; s.Q = s.Qn; s.Qn = t; }
+    if (par & 2u) {
+        uint64_t* t = s.bkey; s.bkey = s.bkey2; s.bkey2 = t;
+        t = s.mask; s.mask = s.mask2; s.mask2 = t;
+        t = s.grown; s.grown = s.grown2; s.grown2 = t;
+    }
+    return s;
+}
 
 // ---- key packing (A18): field j at shift (n-1-j)*bits, biased by 2^(bits-1); dim 0 most significant
 __device__ __forceinline__ int field_shift(const Params& p, int j) { return (p.n - 1 - j) * p.bits; }
@@ -221,10 +239,10 @@ __device__ __forceinline__ double cfl_term(const Params& p, const double ul[NDIM
 }
 
 // monotonised-central limiter, division-free (A3)
-// active table size for NB bricks: room for the brick count to grow 4x before the load factor is
+// active table size for NB bricks: room for the brick count to grow 8x before the load factor is
 // reached, never below 2^16 slots, never above the allocation
 __host__ __device__ __forceinline__ unsigned long long table_slots_for(const Params& p, unsigned long long NB) {
-    unsigned long long want = (unsigned long long)((double)NB * 4.0 / p.load_factor) + 1ull;
+    unsigned long long want = (unsigned long long)((double)NB * 8.0 / p.load_factor) + 1ull;
     if (want < (1ull << 16)) want = 1ull << 16;
     return want < p.slots ? want : p.slots;
 }
@@ -237,10 +255,14 @@ __device__ __forceinline__ double mc_limit(double a, double b) {
 
 // same limiter, cheaper: sign test on the high words instead of a product (differs from mc_limit only
 // when a*b underflows to zero, where the result is below 1e-150 anyway)
+// (plain compare-and-select minimum: the operands are never NaN, and fmin's NaN handling costs ~8
+// instructions per call in SASS)
+__device__ __forceinline__ double dmin(double a, double b) { return a < b ? a : b; }
 __device__ __forceinline__ double mc_limit_fast(double a, double b) {
     if ((__double2hiint(a) ^ __double2hiint(b)) < 0) return 0.0;
-    const double m1 = fmin(fabs(a), fabs(b));
-    const double m = fmin(0.5 * fabs(a + b), m1 + m1);
+    const double fa = fabs(a), fb = fabs(b);
+    const double m1 = dmin(fa, fb);
+    const double m = dmin(0.5 * (fa + fb), m1 + m1);      // same sign: |a + b| = |a| + |b|
     return copysign(m, a);
 }
 
