@@ -153,7 +153,7 @@ def main():
     ap.add_argument("--workload", default="cfg2")
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--run-mode", type=int, default=1, help="gbees_run: 0 = persistent cooperative kernel, 1 = host loop of step/prune launches")
+    ap.add_argument("--run-mode", type=int, default=0, help="gbees_run: 0 = device-side step control (no host round trip per step), 1 = host loop of gbees_step/gbees_prune")
     args = ap.parse_args()
     cfg = workload(args.workload)
     if args.impl == "reference":
@@ -216,17 +216,22 @@ def main():
         phases = {k: {"ms": round(v[0], 4), "launches": v[1],
                       "algo_GBps": (pb.get(k, 0) / (v[0] * 1e-3) / 1e9 if v[0] > 0 else None)}
                   for k, v in prof.items() if v[1]}
-        if args.run_mode == 0:   # one persistent kernel: its bytes are the whole job's
-            phases["run"]["algo_GBps"] = algo_bytes(st_prof, n, alpha) / (phases["run"]["ms"] * 1e-3) / 1e9
-            phases["run"]["inside_ms"] = {k: round(v, 3) for k, v in g.run_breakdown().items()}
         dom = max(phases, key=lambda k: phases[k]["ms"])
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))) if os.path.exists(
             os.path.join(ROOT, "MEASURED_PEAKS.json")) else None
         peak, peak_src = (peaks["hbm_gbs"], "measured") if peaks else (6650.0, "fallback")
         job_GBps = algo_bytes(st, n, alpha) / (ms_tot / args.steps * 1e-3) / 1e9
         dom_GBps = phases[dom]["algo_GBps"] or 0.0
+        # measured DRAM traffic of the dominant kernel, from the committed ncu --set full capture (bytes per cell-update)
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "traffic.json")
+        if os.path.exists(tpath):
+            tj = json.load(open(tpath))
+            if tj.get("phase") == dom and tj.get("workload") == cfg["name"]:
+                traffic = tj["dram_bytes_per_cell_update"] * st_prof["cell_updates"] / max(phases[dom]["launches"], 1)
         roofline = {"bound": "hbm", "kernel": dom, "achieved": dom_GBps, "peak": peak, "unit": "GB/s",
-                    "frac": dom_GBps / peak, "traffic": None, "peak_source": peak_src,
+                    "frac": dom_GBps / peak, "traffic": traffic, "peak_source": peak_src,
+                    "algo_bytes_per_launch": pb.get(dom, 0) / max(phases[dom]["launches"], 1),
                     "whole_job": {"achieved": job_GBps, "frac": job_GBps / peak,
                                   "frac_of_8TBps": job_GBps / 8000.0, "algo_bytes_per_job": algo_bytes(st, n, alpha)},
                     "phases": phases}
