@@ -359,7 +359,13 @@ int gbees_create(gbees_ctx** out, int n, const double* dx, double threshold, int
     p.bits = 63 / n > 31 ? 31 : 63 / n;
     p.bias = 1ll << (p.bits - 1);
     p.hi_res = o.hi_res; p.limiter = o.limiter; p.normalise = !o.no_normalise;
-    for (int j = 0; j < n; ++j) p.h[j] = dx[j];
+    p.h_pow2 = 1;
+    for (int j = 0; j < n; ++j) {
+        p.h[j] = dx[j];
+        p.hinv[j] = 1.0 / dx[j];
+        int e;
+        if (std::frexp(dx[j], &e) != 0.5) p.h_pow2 = 0;     // mantissa 0.5 <=> power of two
+    }
     for (int k = 0; k < need; ++k) p.par[k] = params[k];
     p.thresh = threshold; p.cfl = o.cfl;
     p.max_cells = (uint64_t)o.max_cells;

@@ -135,6 +135,7 @@ __device__ void phase_targets(const Params& p, const Store& st, DevState* ds) {
     __shared__ unsigned long long sEdge[ND];
     __shared__ unsigned long long sQk[GROW ? WPB : 1][GROW ? NT : 1], sQm[GROW ? WPB : 1][GROW ? NT : 1];   // new cells: (brick key, bits)
     __shared__ unsigned sQn[WPB];
+    __shared__ unsigned sQo[GROW ? WPB : 1][GROW ? NT : 1];   // exclusive prefix of the new-cell counts
     if (threadIdx.x < ND) sEdge[threadIdx.x] = edge_mask<NDIM>(threadIdx.x >> 1, threadIdx.x & 1);
     __syncthreads();
     const uint32_t NB0 = GROW ? ds->NB_before_grow : min(ds->NB, p.capB);
@@ -264,25 +265,41 @@ __device__ void phase_targets(const Params& p, const Store& st, DevState* ds) {
             }
         }
         __syncwarp();
-        if (GROW) {   // count the new cells and fold their CFL terms into the running maximum (Eq. 8)
+        if (GROW) {   // count the new cells and fold their CFL terms into the running maximum (Eq. 8):
+            // the queued (brick, bits) pairs are flattened so that every lane takes one new cell at a time
             const unsigned nq = sQn[w];
-            for (unsigned k = 0; k < nq; ++k) {
-                const unsigned long long fresh = sQm[w][k];
-                int32_t TB[NDIM];
-                unpack<NDIM>(p, sQk[w][k], TB);
+            if (nq) {
+                unsigned run = 0;
+                for (unsigned base = 0; base < nq; base += 32) {
+                    const unsigned k = base + lane;
+                    const unsigned cnt = k < nq ? (unsigned)__popcll(sQm[w][k]) : 0u;
+                    unsigned inc = cnt;
 #pragma unroll
-                for (int hh = 0; hh < 2; ++hh) {
-                    const int tl = (int)lane + 32 * hh;
-                    if (!((fresh >> tl) & 1ull)) continue;
-                    int32_t tc[NDIM];
+                    for (int o = 1; o < 32; o <<= 1) {
+                        const unsigned v = __shfl_up_sync(0xffffffffu, inc, o);
+                        if ((int)lane >= o) inc += v;
+                    }
+                    if (k < nq) sQo[w][k] = run + inc - cnt;
+                    run += __shfl_sync(0xffffffffu, inc, 31);
+                }
+                __syncwarp();
+                for (unsigned idx = lane; idx < run; idx += 32) {
+                    unsigned k = 0;
+                    while (k + 1 < nq && sQo[w][k + 1] <= idx) ++k;
+                    unsigned r = idx - sQo[w][k];
+                    unsigned long long mm = sQm[w][k];
+                    while (r--) mm &= mm - 1ull;
+                    const int tl = __ffsll((long long)mm) - 1;
+                    int32_t TB[NDIM], tc[NDIM];
+                    unpack<NDIM>(p, sQk[w][k], TB);
                     cell_coords<NDIM>(TB, tl, tc);
                     double ul[NDIM], uu[NDIM];
                     face_velocities<NDIM, DYN>(p, tc, ul, uu);
                     smax = fmax(smax, cfl_term<NDIM>(p, ul));
                     ++n_new;
                 }
+                __syncwarp();
             }
-            __syncwarp();
         }
     }
     if (GROW) {

@@ -22,6 +22,8 @@ struct Params {
     int normalise;
     int64_t bias;        // 2^(bits-1): cell coordinates live in [-bias, bias-1] (A18)
     double h[MAXN];
+    double hinv[MAXN];   // 1 / h_j
+    int h_pow2;          // every h_j is a power of two: x / h_j == x * hinv_j bit for bit
     double mu[MAXN];     // grid origin
     double par[MAXN * MAXN];
     double thresh;
@@ -234,7 +236,8 @@ template <int NDIM>
 __device__ __forceinline__ double cfl_term(const Params& p, const double ul[NDIM]) {
     double s = 0.0;
 #pragma unroll
-    for (int j = 0; j < NDIM; ++j) s = DADD(s, __ddiv_rn(fabs(ul[j]), p.h[j]));
+    for (int j = 0; j < NDIM; ++j)
+        s = DADD(s, p.h_pow2 ? DMUL(fabs(ul[j]), p.hinv[j]) : __ddiv_rn(fabs(ul[j]), p.h[j]));
     return s;
 }
 
