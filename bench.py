@@ -8,7 +8,7 @@ hot path (grow, dt, CTU flux, update, normalise, prune/compact/rehash) over one 
 (init_gaussian and export outside the timed region); `e2e` = the same jobs timed through the C ABI
 with HOST buffers: init_gaussian(host mean/cov) + run + export into pinned host arrays.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg2|cfg3|cfg3s|cfg0|cfg1] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg2|cfg3|cfg3s|cfg0|cfg1|cfg4] [--impl reference]
 """
 import argparse
 import json
@@ -116,6 +116,20 @@ def drive_oracle(o, cfg, budget_s):
     return upd, time.perf_counter() - t0, k
 
 
+def aggregate(ms, upd, device="cpu"):
+    """Replicas-only multi-GPU: time = max over ranks, work = sum over ranks."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return ms, upd
+    dist.barrier()
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    u = torch.tensor([upd], dtype=torch.float64, device=device)
+    dist.all_reduce(u)
+    return t.item(), u.item()
+
+
 def make_oracle(cfg):
     from oracle.binding import Oracle
     o = Oracle(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfg["cfl"])
@@ -145,6 +159,47 @@ def run_reference(args, cfg):
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}))
 
 
+def run_cfg4(args):
+    """BASELINE config 4: hashtable / compaction microbench (probes/op against PAPER.md:192, M ops/s,
+    modelled GB/s: 16 B slot + 8 B key per insert / successful probe chain, 8 + 1 + 8 B per compacted key)."""
+    import torch
+    from paper_2508_13986_b200 import HashTable, workloads as W
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device: there is no CPU fallback"
+    rows = []
+
+    def timed(fn):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(); e0.record(); r = fn(); e1.record(); e1.synchronize()
+        return r, e0.elapsed_time(e1) * 1e-3
+
+    for K in [int(k) for k in args.cfg4_keys.split(",")]:
+        keys = W.config4_keys(K)
+        rng = np.random.default_rng(W.S0 + 42)
+        dele = torch.from_numpy((rng.random(K) < 0.3).astype(np.uint8)).cuda()
+        unit = np.uint64(1) << (np.uint64(10) * np.arange(6, dtype=np.uint64))
+        sub = keys[:max(K // 12, 1)]
+        q = torch.from_numpy(np.concatenate([sub + u for u in unit] + [sub - u for u in unit]).view(np.int64)).cuda()
+        for alpha in (0.3, 0.4, 0.5, 0.6, 0.7, 0.8):
+            kt = torch.from_numpy(keys.view(np.int64)).cuda()
+            ht = HashTable(int(np.ceil(K / alpha)))
+            idx = torch.empty(K, dtype=torch.int32, device="cuda")
+            qo = torch.empty(q.numel(), dtype=torch.int32, device="cuda")
+            p_ins, t_ins = timed(lambda: ht.insert(kt, idx))
+            p_hit, t_hit = timed(lambda: ht.lookup(kt, idx))
+            p_nb, t_nb = timed(lambda: ht.lookup(q, qo))
+            kept, t_cmp = timed(lambda: ht.compact(kt, dele))
+            ht.close()
+            rows.append({"keys": K, "alpha": alpha,
+                         "insert": {"probes_per_op": p_ins / K, "Mops": K / t_ins / 1e6, "GBps": K * (8 + 16 * p_ins / K + 16) / t_ins / 1e9},
+                         "lookup_hit": {"probes_per_op": p_hit / K, "Mops": K / t_hit / 1e6, "GBps": K * (8 + 16 * p_hit / K + 4) / t_hit / 1e9},
+                         "lookup_neighbours": {"probes_per_op": p_nb / q.numel(), "Mops": q.numel() / t_nb / 1e6,
+                                               "GBps": q.numel() * (8 + 16 * p_nb / q.numel() + 4) / t_nb / 1e9},
+                         "delete30_compact_rebuild": {"survivors": kept, "Mkeys_per_s": K / t_cmp / 1e6}})
+    print(json.dumps({"metric": "hashtable / compaction microbench (BASELINE config 4)", "unit": "probes/op, M ops/s, GB/s",
+                      "n_gpus": 1, "data": "synthetic", "config": {"workload": "cfg4_hashtable", "keys": args.cfg4_keys},
+                      "expected_probes": "PAPER.md:192: hit (1+1/(1-a))/2, miss (1+1/(1-a)^2)/2", "rows": rows}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -153,8 +208,11 @@ def main():
     ap.add_argument("--workload", default="cfg2")
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cfg4-keys", default="1000000,10000000", help="key counts of the cfg4 microbench (1e8 needs ~25 GB)")
     ap.add_argument("--run-mode", type=int, default=0, help="gbees_run: 0 = device-side step control (no host round trip per step), 1 = host loop of gbees_step/gbees_prune")
     args = ap.parse_args()
+    if args.workload == "cfg4":
+        return run_cfg4(args)
     cfg = workload(args.workload)
     if args.impl == "reference":
         return run_reference(args, cfg)
@@ -202,12 +260,7 @@ def main():
             ms_tot, upd_tot, launches = ms_tot + ms, upd_tot + st["cell_updates"], launches + st["launches"]
         torch.cuda.synchronize()
         clocks = sampler.result()
-        if world > 1:
-            dist.barrier()
-            t = torch.tensor([ms_tot], device="cuda"); dist.all_reduce(t, op=dist.ReduceOp.MAX); ms_max = t.item()
-            u = torch.tensor([upd_tot], device="cuda", dtype=torch.float64); dist.all_reduce(u); upd_all = u.item()
-        else:
-            ms_max, upd_all = ms_tot, upd_tot
+        ms_max, upd_all = aggregate(ms_tot, upd_tot, "cuda")
 
         # per-phase CUDA-event timing of one more job (same workload, same launch configuration)
         ms_prof, st_prof = job(profile=True)

@@ -45,14 +45,14 @@ extern "C" {
 typedef struct gbees_ctx gbees_ctx;
 
 typedef struct gbees_opts {
-    int64_t max_cells;   /* pool capacity; hashtable has ceil(max_cells / load_factor) slots */
+    int64_t max_cells;   /* active-cell capacity; storage = max(ceil(max_cells/16), 256) bricks of 64 cell slots, brick hashtable with ceil(bricks / load_factor) slots */
     double load_factor;  /* default 0.5 */
     double cfl;          /* C in dt = C * min_c (sum_j |u_cj| / h_j)^-1, Eq. (8); default 0.9 */
     int hi_res;          /* 1 = add the high-resolution (limited Lax-Wendroff) term; default 1 */
     int limiter;         /* 0 = monotonised central, 1 = none (phi == 1, test mode) */
     int no_grow;         /* test mode: gbees_step does not grow the grid */
     int no_normalise;    /* test mode: keep raw (un-normalised) masses after step / prune */
-    int run_mode;        /* gbees_run: 0 = persistent cooperative kernel (default), 1 = host loop of step/prune */
+    int run_mode;        /* gbees_run: 0 = device-side step control, no host round trip per step (default); 1 = host loop of gbees_step / gbees_prune */
     int device;          /* CUDA device ordinal */
     void* stream;        /* cudaStream_t to run on (e.g. torch's current stream); NULL = default */
 } gbees_opts;
@@ -75,14 +75,14 @@ typedef struct gbees_stats_t {
 
 /* phases of the hot path, for launch accounting and optional CUDA-event timing */
 enum {
-    GBEES_PH_GROW = 0,  /* a1: grow (insert downwind targets) */
-    GBEES_PH_LINK,      /* adjacency of the new cells + their CFL terms (a2/a3) */
-    GBEES_PH_PASSA,     /* a2+a4: face velocities, upwind-owner CTU fluxes */
-    GBEES_PH_PASSB,     /* a5+a6: gather neighbour fluxes, update, mass sum, dt/t bookkeeping */
+    GBEES_PH_GROW = 0,  /* a1: grow (activate downwind targets, create bricks) + CFL terms of the new cells (a3) */
+    GBEES_PH_LINK,      /* adjacency of the bricks created by the grow */
+    GBEES_PH_PASSA,     /* a2+a4: face velocities, upwind-owner CTU fluxes (k_flux1) */
+    GBEES_PH_PASSB,     /* a5+a6: fetch neighbour-brick fluxes, update, mass sum, dt/t bookkeeping (k_flux2) */
     GBEES_PH_MARK,      /* a7: prune marking */
-    GBEES_PH_COMPACT,   /* a7: decoupled-lookback scan + stream compaction */
+    GBEES_PH_COMPACT,   /* a7: decoupled-lookback scan over bricks + row compaction */
     GBEES_PH_REBUILD,   /* a7/a0: hashtable clear + re-insert */
-    GBEES_PH_RELINK,    /* adjacency + CFL maximum for all cells */
+    GBEES_PH_RELINK,    /* adjacency + CFL maximum for all cells, mass sum, renormalise */
     GBEES_PH_SUM,       /* a6: mass sum + renormalise outside a step */
     GBEES_PH_CORRECT,   /* a8 */
     GBEES_PH_RUN,       /* a9: persistent cooperative step loop (whole launch) */
@@ -125,8 +125,10 @@ int gbees_correct(gbees_ctx* ctx, const double* z, const double* R);
  * cap < count: nothing written, *count = needed, GBEES_ERR_BUFFER. count: host pointer. */
 int gbees_export(gbees_ctx* ctx, int32_t* keys, double* p, int64_t cap, int64_t* count);
 
-/* Persistent step loop: advance until t == t_target or max_steps steps, pruning
- * after every prune_every-th step (0 = never). Observationally identical to the same sequence of
+/* Step loop kept on the device: advance until t == t_target or max_steps steps,
+ * pruning after every prune_every-th step (0 = never). The launches of a chunk of steps are enqueued
+ * at once; a device flag set by each step's last block decides whether the next ones execute, so
+ * there is no host round trip per step. Observationally identical to the same sequence of
  * gbees_step(&cap = t_target - t) / gbees_prune calls. steps_done: host, nullable. */
 int gbees_run(gbees_ctx* ctx, double t_target, int64_t max_steps, int prune_every, int64_t* steps_done);
 
@@ -137,10 +139,9 @@ int gbees_stats(gbees_ctx* ctx, gbees_stats_t* out /*host*/);
  * nullable), then switch CUDA-event timing of every phase on/off. Synchronises the stream.
  * Launch counts are always kept; milliseconds only while profiling is enabled. */
 int gbees_profile(gbees_ctx* ctx, int enable, double* phase_ms, int64_t* phase_launches);
-/* Read-and-reset the time spent per phase INSIDE the persistent kernel of gbees_run (device
- * %globaltimer, block 0, each phase including the grid barrier that ends it). Always collected.
- * phase_ms: host [GBEES_PHASES]; COMPACT holds keep-clear + scan + compaction, RELINK the adjacency
- * remap + table clear, REBUILD the re-insert + CFL maximum + mass sum. */
+/* Kept for ABI stability: per-phase device timers of the former persistent kernel. The phases of
+ * gbees_run are separate launches now and are timed by gbees_profile; this call returns zeros.
+ * phase_ms: host [GBEES_PHASES]. */
 int gbees_run_breakdown(gbees_ctx* ctx, double* phase_ms);
 const char* gbees_last_error(gbees_ctx* ctx);
 int gbees_clear_error(gbees_ctx* ctx);

@@ -4,4 +4,4 @@ Every step of the path runs in the hand-written CUDA kernels behind the C ABI of
 this package only marshals arguments. There is no CPU fallback: importing `binding` without the
 built extension raises.
 """
-from .binding import Gbees, GbeesError, lib_path  # noqa: F401
+from .binding import Gbees, GbeesError, HashTable, lib_path  # noqa: F401

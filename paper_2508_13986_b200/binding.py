@@ -190,3 +190,52 @@ class Gbees:
         cnt = C.c_int64()
         self._chk(lib().gbees_export(self._h, keys_t.data_ptr(), p_t.data_ptr(), int(p_t.numel()), C.byref(cnt)))
         return cnt.value
+
+
+class HashTable:
+    """BASELINE config 4: the library's open-addressing table on its own (gbees_ht_* in include/gbees.h).
+    Keys / flags are torch CUDA tensors (int64 holding the packed 64-bit keys, uint8 delete flags)."""
+
+    def __init__(self, slots, device=0):
+        L = lib()
+        vp = C.c_void_p
+        L.gbees_ht_create.argtypes = [C.POINTER(vp), C.c_int64, C.c_int]
+        L.gbees_ht_destroy.argtypes = [vp]
+        L.gbees_ht_insert.argtypes = [vp, vp, C.c_int64, vp, C.POINTER(C.c_uint64)]
+        L.gbees_ht_lookup.argtypes = [vp, vp, C.c_int64, vp, C.POINTER(C.c_uint64)]
+        L.gbees_ht_compact.argtypes = [vp, vp, vp, C.c_int64, C.POINTER(C.c_int64)]
+        self._h = vp()
+        rc = L.gbees_ht_create(C.byref(self._h), int(slots), int(device))
+        if rc:
+            self._h = None
+            raise GbeesError(rc, "gbees_ht_create failed")
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().gbees_ht_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def insert(self, keys_t, idx_out_t=None):
+        pr = C.c_uint64()
+        rc = lib().gbees_ht_insert(self._h, keys_t.data_ptr(), int(keys_t.numel()),
+                                   idx_out_t.data_ptr() if idx_out_t is not None else None, C.byref(pr))
+        if rc:
+            raise GbeesError(rc, "gbees_ht_insert failed")
+        return pr.value
+
+    def lookup(self, query_t, out_t=None):
+        pr = C.c_uint64()
+        rc = lib().gbees_ht_lookup(self._h, query_t.data_ptr(), int(query_t.numel()),
+                                   out_t.data_ptr() if out_t is not None else None, C.byref(pr))
+        if rc:
+            raise GbeesError(rc, "gbees_ht_lookup failed")
+        return pr.value
+
+    def compact(self, keys_t, del_t):
+        k = C.c_int64()
+        rc = lib().gbees_ht_compact(self._h, keys_t.data_ptr(), del_t.data_ptr(), int(keys_t.numel()), C.byref(k))
+        if rc:
+            raise GbeesError(rc, "gbees_ht_compact failed")
+        return k.value

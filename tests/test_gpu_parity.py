@@ -201,3 +201,40 @@ def test_run_persistent_loop_lorenz96_to_time(prune_every):
     assert abs(g.step() - o.step()) <= 1e-14
     g.prune(); o.prune()
     compare_states(*g.export(), *o.export(), cfg["thresh"], 1e-9, what="L96 run + step + prune")
+
+
+def test_config2_full_size_against_oracle_golden():
+    """BASELINE config 2 at full size, in the launch configuration bench.py times (gbees_run, device-side
+    step control): step count, final time, cell counts after every 5th step and the masses of 128
+    sampled cells against the oracle's stored result (tests/golden/cfg2_full_oracle.json, written by
+    tests/golden/make_cfg2_golden.py, which calls only oracle/)."""
+    import json
+    import os
+    gold = json.load(open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "cfg2_full_oracle.json")))
+    cfg = W.config2()
+    g = G(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfg["cfl"], max_cells=cfg["max_cells"])
+    g.init_gaussian(cfg["mean"], cfg["cov"])
+    counts = {0: g.count()}
+    done = 0
+    while g.time() < cfg["t_end"]:                      # chunks of 5 steps so the cell counts can be compared
+        done += g.run(cfg["t_end"], max_steps=5, prune_every=0)
+        if done % cfg["prune_every"] == 0:
+            g.prune()
+        counts[done] = g.count()
+    assert done == gold["steps"]
+    assert g.time() == gold["t"] == cfg["t_end"]
+    for k, cnt in counts.items():
+        assert cnt == gold["cells_after_each_step"][k], f"cell count after step {k}"
+    gk, gp = g.export()
+    assert len(gp) == gold["final_cells"]
+    assert gp.sum() == pytest.approx(1.0, abs=1e-12)
+    lut = {tuple(k): v for k, v in zip(gk.tolist(), gp.tolist())}
+    got = np.array([lut[tuple(k)] for k in gold["sample_keys"]])      # KeyError = active sets differ
+    want = np.array(gold["sample_p"])
+    assert np.max(np.abs(got - want)) <= 1e-8 * gold["p_max"]
+    # and the same job through one gbees_run call gives the same state
+    g2 = G(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfg["cfl"], max_cells=cfg["max_cells"])
+    g2.init_gaussian(cfg["mean"], cfg["cov"])
+    assert g2.run(cfg["t_end"], prune_every=cfg["prune_every"]) == gold["steps"]
+    k2, p2 = g2.export()
+    assert np.array_equal(k2, gk) and np.max(np.abs(p2 - gp)) <= 1e-12 * gp.max()
