@@ -130,7 +130,7 @@ __device__ void phase_targets(const Params& p, const Store& st, DevState* ds) {
     using G = Geo<NDIM>;
     constexpr int ND = 2 * NDIM, NT = ND + 2 * NDIM * (NDIM - 1), OWN = ND;
     __shared__ unsigned long long sO[WPB][ND];        // O_d: sources with outflow through face d
-    __shared__ unsigned long long sT[WPB][ND + 1];    // target bits per destination (face neighbours, own)
+    __shared__ unsigned long long sDiag[WPB][NT - ND > 0 ? NT - ND : 1];   // target bits bound for diagonal bricks, per edge class
     __shared__ uint32_t sAdj[WPB][ND];
     __shared__ unsigned long long sEdge[ND];
     __shared__ unsigned long long sQk[GROW ? WPB : 1][GROW ? NT : 1], sQm[GROW ? WPB : 1][GROW ? NT : 1];   // new cells: (brick key, bits)
@@ -190,7 +190,6 @@ __device__ void phase_targets(const Params& p, const Store& st, DevState* ds) {
         }
         if (!src) continue;
         if (lane < ND) sAdj[w][lane] = st.adj[(size_t)b * ND + lane];
-        if (lane <= ND) sT[w][lane] = (!GROW && lane == OWN) ? src : 0ull;   // mark: sources keep themselves
         if (lane == 0) sQn[w] = 0u;
 #pragma unroll
         for (int d = 0; d < ND; ++d) {
@@ -200,66 +199,83 @@ __device__ void phase_targets(const Params& p, const Store& st, DevState* ds) {
         }
         if (GROW && lane == 0) st.grown[b] = g | src;            // autonomous f: grow once
         __syncwarp();
-        for (int t = (int)lane; t < NT; t += 32) {
-            int j, sj, l2, sl;
-            decode_target<NDIM>(t, j, sj, l2, sl);
-            const int d1 = 2 * j + sj;
-            unsigned long long S = sO[w][d1];
-            if (l2 >= 0) S &= sO[w][2 * l2 + sl];
-            if (!S) continue;
-            const int s1 = 1 << G::SH(j), w1 = G::MK(j) * s1;
-            unsigned long long in = S & ~sEdge[d1], cr = S & sEdge[d1];     // stay in the brick / cross face d1
-            in = sj ? in << s1 : in >> s1;
-            cr = sj ? cr >> w1 : cr << w1;
-            if (l2 < 0) {
-                if (in) atomicOr(&sT[w][OWN], in);
-                if (cr) atomicOr(&sT[w][d1], cr);
-                continue;
-            }
-            const int d2 = 2 * l2 + sl;
-            const int s2 = 1 << G::SH(l2), w2 = G::MK(l2) * s2;
-            const unsigned long long e2 = sEdge[d2];
-            unsigned long long p00 = in & ~e2, p01 = in & e2, p10 = cr & ~e2, p11 = cr & e2;
-            p00 = sl ? p00 << s2 : p00 >> s2;
-            p10 = sl ? p10 << s2 : p10 >> s2;
-            p01 = sl ? p01 >> w2 : p01 << w2;
-            p11 = sl ? p11 >> w2 : p11 << w2;
-            if (p00) atomicOr(&sT[w][OWN], p00);
-            if (p01) atomicOr(&sT[w][d2], p01);
-            if (p10) atomicOr(&sT[w][d1], p10);
-            if (p11) {   // diagonal brick: through the adjacency of either face neighbour, else by key
-                uint32_t row = NBR_NONE;
-                const uint32_t r1 = sAdj[w][d1], r2 = sAdj[w][d2];
-                if (r1 != NBR_NONE) row = st.adj[(size_t)r1 * ND + d2];
-                if (row == NBR_NONE && r2 != NBR_NONE) row = st.adj[(size_t)r2 * ND + d1];
-                const uint64_t u1 = 1ull << ((NDIM - 1 - j) * p.bits), u2 = 1ull << ((NDIM - 1 - l2) * p.bits);
-                uint64_t key = sj ? bk + u1 : bk - u1;
-                key = sl ? key + u2 : key - u2;
-                if (GROW) {
-                    account(key, grow_apply(p, st, ds, NB0, slots, ND, row, key, p11));
-                } else {
-                    if (row == NBR_NONE) row = ht_find(st.table, slots, key);
-                    if (row != NBR_NONE) {
-                        const unsigned long long x = p11 & st.mask[row];
-                        if (x) atomicOr((unsigned long long*)&st.keep[row], x);
-                    }
+        // ---- target classes: shift the source masks to the target slots, split by destination brick.
+        // No atomics here: the parts bound for the own brick and the 2n face neighbours are merged
+        // across the lanes with warp OR-reductions (lane d keeps destination d); a diagonal part is
+        // parked in shared memory under its class number.
+        unsigned long long myT = (!GROW && lane == OWN) ? src : 0ull;   // mark: sources keep themselves
+#pragma unroll
+        for (int it = 0; it < (NT + 31) / 32; ++it) {
+            const int t = (int)lane + 32 * it;
+            unsigned long long vOwn = 0ull, v1 = 0ull, v2 = 0ull;
+            int d1 = -1, d2 = -1;
+            if (t < NT) {
+                int j, sj, l2, sl;
+                decode_target<NDIM>(t, j, sj, l2, sl);
+                d1 = 2 * j + sj;
+                unsigned long long S = sO[w][d1];
+                if (l2 >= 0) S &= sO[w][2 * l2 + sl];
+                const int s1 = 1 << G::SH(j), w1 = G::MK(j) * s1;
+                unsigned long long in = S & ~sEdge[d1], cr = S & sEdge[d1];     // stay in the brick / cross face d1
+                in = sj ? in << s1 : in >> s1;
+                cr = sj ? cr >> w1 : cr << w1;
+                if (l2 < 0) { vOwn = in; v1 = cr; }
+                else {
+                    d2 = 2 * l2 + sl;
+                    const int s2 = 1 << G::SH(l2), w2 = G::MK(l2) * s2;
+                    const unsigned long long e2 = sEdge[d2];
+                    unsigned long long p00 = in & ~e2, p01 = in & e2, p10 = cr & ~e2, p11 = cr & e2;
+                    vOwn = sl ? p00 << s2 : p00 >> s2;
+                    v1 = sl ? p10 << s2 : p10 >> s2;
+                    v2 = sl ? p01 >> w2 : p01 << w2;
+                    sDiag[w][t - ND] = sl ? p11 >> w2 : p11 << w2;
                 }
+            }
+            if (!__any_sync(0xffffffffu, (vOwn | v1 | v2) != 0ull)) continue;
+#pragma unroll
+            for (int d = 0; d <= ND; ++d) {
+                const unsigned long long x = d == OWN ? vOwn : ((d == d1 ? v1 : 0ull) | (d == d2 ? v2 : 0ull));
+                const unsigned lo32 = __reduce_or_sync(0xffffffffu, (unsigned)x);
+                const unsigned hi32 = __reduce_or_sync(0xffffffffu, (unsigned)(x >> 32));
+                if ((int)lane == d) myT |= ((unsigned long long)hi32 << 32) | lo32;
             }
         }
         __syncwarp();
-        if (lane <= ND) {   // one lane per destination: own brick and the 2n face neighbours
-            const unsigned long long T = sT[w][lane];
-            if (T) {
-                const uint32_t row = lane == OWN ? b : sAdj[w][lane];
-                if (GROW) {
-                    uint64_t key = bk;
-                    if (lane != OWN) {
-                        const uint64_t u1 = 1ull << ((NDIM - 1 - (int)(lane >> 1)) * p.bits);
-                        key = (lane & 1) ? bk + u1 : bk - u1;
-                    }
-                    account(key, grow_apply(p, st, ds, NB0, slots, ND, row, key, T));
-                } else if (row != NBR_NONE) {
-                    const unsigned long long x = T & st.mask[row];
+        // ---- apply: lane d <= 2n takes destination d; then the diagonal parts, one lane per class
+        if (lane <= ND && myT) {
+            const uint32_t row = lane == OWN ? b : sAdj[w][lane];
+            if (GROW) {
+                uint64_t key = bk;
+                if (lane != OWN) {
+                    const uint64_t u1 = 1ull << ((NDIM - 1 - (int)(lane >> 1)) * p.bits);
+                    key = (lane & 1) ? bk + u1 : bk - u1;
+                }
+                account(key, grow_apply(p, st, ds, NB0, slots, ND, row, key, myT));
+            } else if (row != NBR_NONE) {
+                const unsigned long long x = myT & st.mask[row];
+                if (x) atomicOr((unsigned long long*)&st.keep[row], x);
+            }
+        }
+        for (int t = ND + (int)lane; t < NT; t += 32) {
+            const unsigned long long p11 = sDiag[w][t - ND];
+            if (!p11) continue;
+            int j, sj, l2, sl;
+            decode_target<NDIM>(t, j, sj, l2, sl);
+            const int d1 = 2 * j + sj, d2 = 2 * l2 + sl;
+            // diagonal brick: through the adjacency of either face neighbour, else by key
+            uint32_t row = NBR_NONE;
+            const uint32_t r1 = sAdj[w][d1], r2 = sAdj[w][d2];
+            if (r1 != NBR_NONE) row = st.adj[(size_t)r1 * ND + d2];
+            if (row == NBR_NONE && r2 != NBR_NONE) row = st.adj[(size_t)r2 * ND + d1];
+            const uint64_t u1 = 1ull << ((NDIM - 1 - j) * p.bits), u2 = 1ull << ((NDIM - 1 - l2) * p.bits);
+            uint64_t key = sj ? bk + u1 : bk - u1;
+            key = sl ? key + u2 : key - u2;
+            if (GROW) {
+                account(key, grow_apply(p, st, ds, NB0, slots, ND, row, key, p11));
+            } else {
+                if (row == NBR_NONE) row = ht_find(st.table, slots, key);
+                if (row != NBR_NONE) {
+                    const unsigned long long x = p11 & st.mask[row];
                     if (x) atomicOr((unsigned long long*)&st.keep[row], x);
                 }
             }
