@@ -63,19 +63,46 @@ __global__ void __launch_bounds__(TPB) k_finish(GP, unsigned nparts, int mode, i
     finish_sum(q, st, ds, nparts, false);
     if (guard == 2 && threadIdx.x == 0) begin_step(ds);   // the prune changed N / NB: refresh the next step's setup
 }
-// prune prologue: clear the marks and the scan descriptors (sizes are only known on the device)
-__global__ void __launch_bounds__(TPB) k_prune_prep(GP) {
+__global__ void __launch_bounds__(TPB) k_prune_scan(GP) { GUARD(2); ST; phase_prune_scan(p, st, ds); }
+__global__ void __launch_bounds__(TPB) k_prune_move(GP) { GUARD(2); ST; phase_prune_move(p, st, ds); }
+// after the move: unused rows back to zero, and the marks / scan descriptors back to zero for the
+// next prune (invariant: keep[] and tile_state[] are all-zero outside a prune)
+__global__ void __launch_bounds__(TPB) k_zero_tail(GP) {
     GUARD(2);
     ST;
+    phase_zero_tail(p, st, ds);
     const uint32_t NB = min(ds->NB, p.capB);
     for (uint32_t i = gtid(); i < NB; i += gthreads()) st.keep[i] = 0ull;
     const uint32_t ntiles = (NB + SCAN_TILE - 1) / SCAN_TILE + 1;
     for (uint32_t i = gtid(); i < ntiles; i += gthreads()) st.tile_state[i] = 0ull;
-    if (gtid() == 0) ds->tile_counter = 0u;
 }
-__global__ void __launch_bounds__(TPB) k_prune_scan(GP) { GUARD(2); ST; phase_prune_scan(p, st, ds); }
-__global__ void __launch_bounds__(TPB) k_prune_move(GP) { GUARD(2); ST; phase_prune_move(p, st, ds); }
-__global__ void __launch_bounds__(TPB) k_zero_tail(GP) { GUARD(2); ST; phase_zero_tail(p, st, ds); }
+// prune tail, one launch: re-insert the brick keys, CFL maximum, mass sum + cell count
+template <int NDIM, int DYN>
+__global__ void __launch_bounds__(TPB) k_prune_tail(GP) {
+    GUARD(2);
+    ST;
+    phase_rebuild(p, st, ds);
+    phase_smax<NDIM, DYN>(p, st, ds);
+    phase_sum(p, st, ds, true);
+}
+// adjacency of all bricks; the last block to finish renormalises and sets up the next step
+template <int NDIM>
+__global__ void __launch_bounds__(TPB) k_link_finish(GP, unsigned nparts) {
+    GUARD(2);
+    ST;
+    __shared__ bool s_last;
+    phase_link<NDIM, true>(p, st, ds);
+    if (threadIdx.x == 0) {
+        __threadfence();
+        s_last = atomicAdd(&ds->ticket, 1u) == gridDim.x - 1;
+    }
+    __syncthreads();
+    if (s_last) {
+        __threadfence();
+        finish_sum(p, st, ds, nparts, false);
+        if (threadIdx.x == 0) { ds->ticket = 0; begin_step(ds); }
+    }
+}
 // after the move: survivors live in Qn and in the second metadata buffers -> flip both parities
 __global__ void k_after_compact(const __grid_constant__ Params p, DevState* ds) {
     GUARD(2);
@@ -406,6 +433,8 @@ int gbees_create(gbees_ctx** out, int n, const double* dx, double threshold, int
     if (cudaMallocHost((void**)&c->h_st, sizeof(DevState)) != cudaSuccess) return bail(GBEES_ERR_CUDA, "cudaMallocHost");
     cudaMemsetAsync(st.Q, 0, cb * 512, c->stream);
     cudaMemsetAsync(st.Qn, 0, cb * 512, c->stream);
+    cudaMemsetAsync(st.keep, 0, cb * 8, c->stream);                                    // all-zero outside a prune
+    cudaMemsetAsync(st.tile_state, 0, (size_t)(c->ntiles_max + 1) * 8, c->stream);
     std::memset(c->h_st, 0, sizeof(DevState));
     c->h_st->scale = 1.0;
     c->h_st->slots = p.slots;
@@ -520,34 +549,23 @@ static int enqueue_step(gbees_ctx* c) {
 
 // enqueue the launches of one prune (each runs only if the device's prune_ok flag is set)
 static int enqueue_prune(gbees_ctx* c) {
-    int rc = GBEES_OK;
-    phase(c, GBEES_PH_MARK, 2, [&] {
-        k_prune_prep<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
-        rc = dispatch(c, [&](auto N_, auto D_) {
-            k_mark<decltype(N_)::value, decltype(D_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
-            return GBEES_OK;
+    int rc = dispatch(c, [&](auto N_, auto D_) {
+        constexpr int NN = decltype(N_)::value, DD = decltype(D_)::value;
+        phase(c, GBEES_PH_MARK, 1, [&] { k_mark<NN, DD><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st); });
+        phase(c, GBEES_PH_COMPACT, 4, [&] {
+            k_prune_scan<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
+            k_prune_move<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
+            k_zero_tail<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
+            k_after_compact<<<1, 1, 0, c->stream>>>(c->p, c->d_st);
         });
+        phase(c, GBEES_PH_REBUILD, 2, [&] {
+            k_clear_table<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 2);
+            k_prune_tail<NN, DD><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
+        });
+        phase(c, GBEES_PH_RELINK, 1, [&] { k_link_finish<NN><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, c->grid); });
+        return GBEES_OK;
     });
     if (rc) return fail(c, rc, "unsupported (n, dynamics) pair");
-    phase(c, GBEES_PH_COMPACT, 4, [&] {
-        k_prune_scan<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
-        k_prune_move<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
-        k_zero_tail<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
-        k_after_compact<<<1, 1, 0, c->stream>>>(c->p, c->d_st);
-    });
-    phase(c, GBEES_PH_REBUILD, 2, [&] {
-        k_clear_table<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 2);
-        k_rebuild<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 2);
-    });
-    phase(c, GBEES_PH_RELINK, 4, [&] {
-        rc = dispatch(c, [&](auto N_, auto D_) {
-            k_link<decltype(N_)::value, true><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 2);
-            k_smax<decltype(N_)::value, decltype(D_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 2);
-            return GBEES_OK;
-        });
-        k_sum<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 1, 2);
-        k_finish<<<1, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, c->grid, 1, 2);
-    });
     return GBEES_OK;
 }
 

@@ -144,7 +144,8 @@ __device__ void phase_targets(const Params& p, const Store& st, DevState* ds) {
     const int32_t lo = (int32_t)(-p.bias), hi = (int32_t)(p.bias - 1);
     const unsigned w = threadIdx.x >> 5, lane = lane_id();
     unsigned long long n_new = 0;
-    double smax = 0.0;
+    const double smax0 = GROW ? __longlong_as_double((long long)ds->smax_bits) : 0.0;   // the maximum so far: most new cells stay below it
+    double smax = smax0;
     // new cells (GROW) are queued per warp as (brick key, bits) and expanded by all lanes below
     auto account = [&](uint64_t key, unsigned long long fresh) {
         if (!fresh) return;
@@ -311,7 +312,7 @@ __device__ void phase_targets(const Params& p, const Store& st, DevState* ds) {
                     cell_coords<NDIM>(TB, tl, tc);
                     double ul[NDIM], uu[NDIM];
                     face_velocities<NDIM, DYN>(p, tc, ul, uu);
-                    smax = fmax(smax, cfl_term<NDIM>(p, ul));
+                    cfl_fold<NDIM>(p, ul, smax);
                     ++n_new;
                 }
                 __syncwarp();
@@ -323,7 +324,7 @@ __device__ void phase_targets(const Params& p, const Store& st, DevState* ds) {
         smax = block_max(smax);
         if (threadIdx.x == 0) {
             if (nn > 0.0) atomicAdd(&ds->N, (unsigned long long)nn);
-            if (smax > 0.0) atomicMax(&ds->smax_bits, (unsigned long long)__double_as_longlong(smax));
+            if (smax > smax0) atomicMax(&ds->smax_bits, (unsigned long long)__double_as_longlong(smax));
         }
     }
 }
@@ -374,7 +375,7 @@ __device__ void phase_smax(const Params& p, const Store& st, DevState* ds) {
         cell_coords<NDIM>(B, l, c);
         double ul[NDIM], uu[NDIM];
         face_velocities<NDIM, DYN>(p, c, ul, uu);
-        smax = fmax(smax, cfl_term<NDIM>(p, ul));
+        cfl_fold<NDIM>(p, ul, smax);
     }
     smax = block_max(smax);
     if (threadIdx.x == 0 && smax > 0.0) atomicMax(&ds->smax_bits, (unsigned long long)__double_as_longlong(smax));

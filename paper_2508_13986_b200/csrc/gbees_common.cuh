@@ -241,6 +241,18 @@ __device__ __forceinline__ double cfl_term(const Params& p, const double ul[NDIM
     return s;
 }
 
+// Fold the CFL term of one cell into a running maximum without paying n true divisions per cell:
+// s~ = sum_j |u_j| * (1/h_j) differs from the exact term by a few ulp, and only a cell whose s~ comes
+// within 1e-12 (relative) of the running maximum can raise it, so the exact term is evaluated for
+// those cells only. The maximum that comes out is the exact one, bit for bit.
+template <int NDIM>
+__device__ __forceinline__ void cfl_fold(const Params& p, const double ul[NDIM], double& best) {
+    double sa = 0.0;
+#pragma unroll
+    for (int j = 0; j < NDIM; ++j) sa = fma(fabs(ul[j]), p.hinv[j], sa);
+    if (sa >= best * (1.0 - 1e-12)) best = fmax(best, cfl_term<NDIM>(p, ul));
+}
+
 // monotonised-central limiter, division-free (A3)
 // active table size for NB bricks: room for the brick count to grow 8x before the load factor is
 // reached, never below 2^16 slots, never above the allocation
