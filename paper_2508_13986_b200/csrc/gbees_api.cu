@@ -150,6 +150,7 @@ struct gbees_ctx {
     int device = 0;
     int sms = 148;
     unsigned grid = 148 * 8;
+    unsigned grid_flux1 = 148 * 2;   // pass 1 (128 registers: 2 resident blocks per SM)
     unsigned ntiles_max = 0;
     size_t stage_bytes = 0;      // size of the phi array (staging area of import / host export)
     int sticky = 0;
@@ -412,6 +413,7 @@ int gbees_create(gbees_ctx** out, int n, const double* dx, double threshold, int
     if ((e = cudaGetDeviceProperties(&prop, c->device)) != cudaSuccess) return bail(GBEES_ERR_CUDA, cudaGetErrorString(e));
     c->sms = prop.multiProcessorCount;
     c->grid = (unsigned)c->sms * 8u;
+    c->grid_flux1 = (unsigned)c->sms * 2u;     // = resident blocks at 128 registers: a persistent grid-stride grid (measured best of 2/4/8/16)
     c->ntiles_max = (p.capB + SCAN_TILE - 1) / SCAN_TILE;
     const size_t cb = p.capB, nd = 2 * (size_t)n;
     auto alloc = [&](void** ptr, size_t bytes) {
@@ -537,8 +539,8 @@ static int enqueue_step(gbees_ctx* c) {
                 cudaFuncSetAttribute(k_flux1<NN, DD, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
                 attr_set = true;
             }
-            if (c->p.hi_res && !c->p.limiter) k_flux1<NN, DD, true><<<c->grid, TPB, smem, c->stream>>>(c->p, c->st, c->d_st);
-            else k_flux1<NN, DD, false><<<c->grid, TPB, smem, c->stream>>>(c->p, c->st, c->d_st);
+            if (c->p.hi_res && !c->p.limiter) k_flux1<NN, DD, true><<<c->grid_flux1, TPB, smem, c->stream>>>(c->p, c->st, c->d_st);
+            else k_flux1<NN, DD, false><<<c->grid_flux1, TPB, smem, c->stream>>>(c->p, c->st, c->d_st);
         });
         phase(c, GBEES_PH_PASSB, 1, [&] { k_flux2<NN><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st); });
         return GBEES_OK;
