@@ -9,6 +9,8 @@
 #include <vector>
 
 #include "../../include/gbees.h"
+#include <cooperative_groups.h>
+
 #include "gbees_brick.cuh"
 
 using namespace gbees;
@@ -67,15 +69,14 @@ __global__ void __launch_bounds__(TPB) k_prune_scan(GP) { GUARD(2); ST; phase_pr
 __global__ void __launch_bounds__(TPB) k_prune_move(GP) { GUARD(2); ST; phase_prune_move(p, st, ds); }
 // after the move: unused rows back to zero, and the marks / scan descriptors back to zero for the
 // next prune (invariant: keep[] and tile_state[] are all-zero outside a prune)
-__global__ void __launch_bounds__(TPB) k_zero_tail(GP) {
-    GUARD(2);
-    ST;
+__device__ __forceinline__ void phase_zero_after_move(const Params& p, const Store& st, DevState* ds) {
     phase_zero_tail(p, st, ds);
     const uint32_t NB = min(ds->NB, p.capB);
     for (uint32_t i = gtid(); i < NB; i += gthreads()) st.keep[i] = 0ull;
     const uint32_t ntiles = (NB + SCAN_TILE - 1) / SCAN_TILE + 1;
     for (uint32_t i = gtid(); i < ntiles; i += gthreads()) st.tile_state[i] = 0ull;
 }
+__global__ void __launch_bounds__(TPB) k_zero_tail(GP) { GUARD(2); ST; phase_zero_after_move(p, st, ds); }
 // prune tail, one launch: re-insert the brick keys, CFL maximum, mass sum + cell count
 template <int NDIM, int DYN>
 __global__ void __launch_bounds__(TPB) k_prune_tail(GP) {
@@ -104,8 +105,7 @@ __global__ void __launch_bounds__(TPB) k_link_finish(GP, unsigned nparts) {
     }
 }
 // after the move: survivors live in Qn and in the second metadata buffers -> flip both parities
-__global__ void k_after_compact(const __grid_constant__ Params p, DevState* ds) {
-    GUARD(2);
+__device__ __forceinline__ void after_compact(const Params& p, DevState* ds) {
     ds->prune_scanned += ds->N;
     ds->prunes += 1;
     ds->NB = ds->NB_after_prune;
@@ -115,6 +115,68 @@ __global__ void k_after_compact(const __grid_constant__ Params p, DevState* ds) 
     ds->N = 0ull;                      // recounted by k_sum
     ds->tile_counter = 0u;
     ds->parity ^= 3u;
+}
+__global__ void k_after_compact(const __grid_constant__ Params p, DevState* ds) { GUARD(2); after_compact(p, ds); }
+
+// ---- a9: persistent step loop for SMALL grids -----------------------------------
+// While the grid has at most a few hundred bricks a step is pure launch / barrier latency (the paper
+// found the same: all its GPUs tie on Lorenz '63). Then the whole loop -- grow, link, pass 1, pass 2,
+// prune -- runs in ONE launch of a single thread-block cluster; the hardware cluster barrier
+// (barrier.cluster, which also invalidates L1) separates the phases instead of kernel boundaries.
+// Same phases, same order, same arithmetic as the stream of launches; leaves the loop when the run
+// is over or the grid has outgrown the cluster (the host then goes on with the launches).
+template <int NDIM, int DYN, bool FAST>
+__global__ void __launch_bounds__(TPB) k_run_small(GP, int prune_every, int no_grow, unsigned long long k_start, uint32_t nb_limit) {
+    namespace cg = cooperative_groups;
+    cg::cluster_group cl = cg::this_cluster();
+    __shared__ bool s_last;
+    unsigned long long k = k_start;
+    for (;;) {
+        cl.sync();
+        if (!ds->go || ds->NB > nb_limit) break;        // uniform: nothing writes these before the next barrier
+        Store st = resolve(st_in, ds);
+        if (!no_grow) {
+            phase_targets<NDIM, DYN, true>(p, st, ds);
+            cl.sync();
+            phase_link<NDIM, false>(p, st, ds);
+            cl.sync();
+        }
+        phase_flux1<NDIM, DYN, FAST>(p, st, ds);
+        cl.sync();
+        phase_flux2_finish<NDIM>(p, st, ds);
+        ++k;
+        if (prune_every <= 0 || k % (unsigned long long)prune_every != 0) continue;
+        cl.sync();
+        st = resolve(st_in, ds);                         // the step flipped the Q / Qn parity
+        phase_targets<NDIM, DYN, false>(p, st, ds);
+        cl.sync();
+        phase_prune_scan(p, st, ds);
+        cl.sync();
+        phase_prune_move(p, st, ds);
+        cl.sync();
+        phase_zero_after_move(p, st, ds);
+        cl.sync();
+        if (gtid() == 0) after_compact(p, ds);
+        cl.sync();
+        st = resolve(st_in, ds);                         // survivors live in the other buffers now
+        phase_clear_table(st, ds);
+        cl.sync();
+        phase_rebuild(p, st, ds);
+        phase_smax<NDIM, DYN>(p, st, ds);
+        phase_sum(p, st, ds, true);
+        cl.sync();
+        phase_link<NDIM, true>(p, st, ds);
+        if (threadIdx.x == 0) {
+            __threadfence();
+            s_last = atomicAdd(&ds->ticket, 1u) == gridDim.x - 1;
+        }
+        __syncthreads();
+        if (s_last) {
+            __threadfence();
+            finish_sum(p, st, ds, gridDim.x, false);
+            if (threadIdx.x == 0) { ds->ticket = 0; begin_step(ds); }
+        }
+    }
 }
 // resize the active table for the current brick count; recount = also reset N and the CFL maximum
 __global__ void k_set_slots(const __grid_constant__ Params p, DevState* ds, int recount) {
@@ -155,7 +217,8 @@ struct gbees_ctx {
     size_t stage_bytes = 0;      // size of the phi array (staging area of import / host export)
     int sticky = 0;
     int no_grow = 0;
-    int run_mode = 0;            // 0 = persistent cooperative kernel, 1 = host loop over step/prune
+    int run_mode = 0;            // 0 = device-side step control, 1 = host loop over step/prune
+    int small_ok = 1;            // the single-cluster persistent loop can be launched on this device
     int run_blocks_per_sm = 0;
     int64_t n_inserted = 0, n_pruned = 0;
     std::string err;
@@ -669,6 +732,31 @@ int gbees_export(gbees_ctx* c, int32_t* keys, double* pv, int64_t cap, int64_t* 
     return GBEES_OK;
 }
 
+// small grids: the whole loop in one launch of a single 8-block cluster (k_run_small)
+constexpr uint32_t SMALL_NB_ENTER = 256, SMALL_NB_LEAVE = 512;
+static int launch_small(gbees_ctx* c, int prune_every, unsigned long long k_start) {
+    int rc = dispatch(c, [&](auto N_, auto D_) {
+        constexpr int NN = decltype(N_)::value, DD = decltype(D_)::value;
+        constexpr size_t smem = sizeof(Flux1Smem<NN>) * WPB;
+        const bool fast = c->p.hi_res && !c->p.limiter;
+        auto kern = fast ? k_run_small<NN, DD, true> : k_run_small<NN, DD, false>;
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return GBEES_ERR_CUDA;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(8); cfg.blockDim = dim3(TPB); cfg.dynamicSmemBytes = smem; cfg.stream = c->stream;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = 8; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        cudaError_t e = cudaSuccess;
+        phase(c, GBEES_PH_RUN, 1, [&] {
+            e = cudaLaunchKernelEx(&cfg, kern, c->p, c->st, c->d_st, prune_every, c->no_grow, k_start, SMALL_NB_LEAVE);
+        });
+        return e == cudaSuccess ? GBEES_OK : GBEES_ERR_CUDA;
+    });
+    if (rc == GBEES_ERR_CUDA) { cudaGetLastError(); c->small_ok = 0; }   // not launchable here: use the launches
+    return rc;
+}
+
 // host loop over gbees_step / gbees_prune with a host round trip per call (opts.run_mode = 1)
 static int run_host_loop(gbees_ctx* c, double t_target, int64_t max_steps, int prune_every, int64_t* steps_done) {
     int64_t k = 0;
@@ -702,6 +790,16 @@ int gbees_run(gbees_ctx* c, double t_target, int64_t max_steps, int prune_every,
     int rc = GBEES_OK;
     int64_t k = 0;     // steps enqueued
     for (;;) {
+        if (c->small_ok && !c->profile && c->h_st->NB <= SMALL_NB_ENTER) {
+            const int lrc = launch_small(c, prune_every, (unsigned long long)k);
+            if (lrc == GBEES_OK) {
+                if ((rc = sync_state(c))) break;
+                k = (int64_t)(c->h_st->steps - steps0);
+                if (!c->h_st->go || k >= max_steps) break;
+                if (c->h_st->NB <= SMALL_NB_ENTER) c->small_ok = 0;   // left the loop for another reason: do not spin
+                else continue;
+            } else if (lrc != GBEES_ERR_CUDA) return fail(c, lrc, "unsupported (n, dynamics) pair");
+        }
         int64_t chunk = 16;
         if (c->h_st->dt > 0.0 && t_target < 1e299) {     // do not enqueue far past the expected end
             const double est = (t_target - c->h_st->t) / c->h_st->dt;
