@@ -22,6 +22,7 @@ def lib():
         L.gbeeso_step.argtypes = [vp, dp]
         L.gbeeso_prune.argtypes = [vp]
         L.gbeeso_correct.argtypes = [vp, dp, dp]
+        L.gbeeso_correct_linear.argtypes = [vp, dp, C.c_int, dp, dp]
         L.gbeeso_export.argtypes = [vp, ip, dp, C.c_int64, C.POINTER(C.c_int64)]
         L.gbeeso_count.argtypes = [vp]
         L.gbeeso_count.restype = C.c_int64
@@ -99,6 +100,13 @@ class Oracle:
         _, zp = _d(z)
         _, rp = _d(R)
         _chk(lib().gbeeso_correct(self._h, zp, rp), "correct")
+
+    def correct_linear(self, H, y, R):
+        """Eq. (4) with y = H x + v (H m x n row-major, R m x m)."""
+        Ha, hp = _d(H)
+        ya, yp = _d(y)
+        _, rp = _d(R)
+        _chk(lib().gbeeso_correct_linear(self._h, hp, int(ya.size), yp, rp), "correct_linear")
 
     def count(self):
         return int(lib().gbeeso_count(self._h))

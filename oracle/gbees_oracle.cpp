@@ -495,6 +495,27 @@ int correct(Oracle& o, const double* z, const double* Rm) {
     return normalise(o);
 }
 
+// ---- f2: Eq. (4) with a linear measurement model y = H x + v, v ~ N(0, R), H m x n.
+// The paper's own scenario observes one state only (y = x3, sigma_y = 1): H = (0 0 1).
+// P_c <- P_c * exp(-1/2 (y - H x_c)^T R^-1 (y - H x_c)), then normalise.
+int correct_linear(Oracle& o, const double* H, int m, const double* y, const double* Rm) {
+    const int n = o.n;
+    if (m < 1 || m > MAXN) return -1;
+    double inv[MAXN * MAXN], det;
+    if (!spd_inverse(m, Rm, inv, &det)) return -3;
+    for (size_t i = 0; i < o.key.size(); ++i) {
+        double x[MAXN], d[MAXN];
+        for (int j = 0; j < n; ++j) x[j] = o.mu[j] + (double)o.key[i][j] * o.h[j];
+        for (int r = 0; r < m; ++r) {
+            double hx = 0.0;
+            for (int j = 0; j < n; ++j) hx += H[r * n + j] * x[j];
+            d[r] = y[r] - hx;
+        }
+        o.P[i] *= std::exp(-0.5 * quad_form(m, inv, d));
+    }
+    return normalise(o);
+}
+
 }  // namespace
 
 // ================================ C ABI (host pointers only) ====================================
@@ -556,6 +577,9 @@ int gbeeso_import(void* h, const double* origin, const int32_t* keys, const doub
 int gbeeso_step(void* h, double* dt) { return step(*(Oracle*)h, dt); }
 int gbeeso_prune(void* h) { return prune(*(Oracle*)h); }
 int gbeeso_correct(void* h, const double* z, const double* R) { return correct(*(Oracle*)h, z, R); }
+int gbeeso_correct_linear(void* h, const double* H, int m, const double* y, const double* R) {
+    return correct_linear(*(Oracle*)h, H, m, y, R);
+}
 
 int gbeeso_export(void* h, int32_t* keys, double* p, int64_t cap, int64_t* count) {
     Oracle* o = (Oracle*)h;

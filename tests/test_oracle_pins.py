@@ -317,6 +317,35 @@ def test_P10_correction_direct_and_kalman():
     assert np.abs(S - (np.eye(n) - K) @ cov0).max() < 5e-3
 
 
+def test_P10b_partial_state_correction_direct_and_kalman():
+    """f2: y = H x + v with the paper's single-state measurement (y = x3) and a 2 x 3 H.
+    Direct definition of Eq. (4), Kalman posterior on the grid, and H = I reduces to correct()."""
+    n, dx = 3, 0.2
+    mu0, cov0 = np.array([-11.5, -10, 9.5]), np.array([[1.0, 0.3, 0.0], [0.3, 0.5, -0.1], [0.0, -0.1, 0.8]])
+    for H, y, R in [(np.array([[0.0, 0.0, 1.0]]), np.array([9.1]), np.array([[1.0]])),
+                    (np.array([[1.0, 0.0, 0.5], [0.0, 2.0, -1.0]]), np.array([-6.9, -29.2]), np.array([[0.9, 0.2], [0.2, 1.4]]))]:
+        o = Oracle(n, [dx] * n, 1e-9, 0, [10, 8 / 3, 28])
+        o.init_gaussian(mu0, cov0)
+        keys, p0 = o.export()
+        o.correct_linear(H, y, R)
+        k1, p1 = o.export()
+        assert np.array_equal(keys, k1)
+        x = mu0 + keys * dx
+        d = y - x @ H.T
+        L = np.exp(-0.5 * np.einsum("ij,jk,ik->i", d, np.linalg.inv(R), d))
+        want = p0 * L / (p0 * L).sum()
+        assert np.max(np.abs(p1 - want)) <= 1e-13 * want.max()
+        K = cov0 @ H.T @ np.linalg.inv(H @ cov0 @ H.T + R)
+        m, S = _moments(keys, p1, mu0, np.array([dx] * n))
+        assert np.abs(m - (mu0 + K @ (y - H @ mu0))).max() < 3e-3
+        assert np.abs(S - (np.eye(n) - K @ H) @ cov0).max() < 6e-3
+    # H = I: identical to the full-state correction
+    z, R = np.array([-11.0, -10.4, 9.9]), np.array([[1.0, 0.2, 0], [0.2, 0.7, 0.1], [0, 0.1, 1.2]])
+    a = Oracle(n, [dx] * n, 1e-9, 0, [10, 8 / 3, 28]); a.init_gaussian(mu0, cov0); a.correct(z, R)
+    b = Oracle(n, [dx] * n, 1e-9, 0, [10, 8 / 3, 28]); b.init_gaussian(mu0, cov0); b.correct_linear(np.eye(3), z, R)
+    assert np.array_equal(a.export()[1], b.export()[1])
+
+
 def test_A8_init_gaussian_set_and_values():
     n, dx, thr = 3, 0.5, 2e-5
     cov = np.array([[1.0, 0.3, 0.0], [0.3, 0.8, -0.2], [0.0, -0.2, 1.1]])
