@@ -120,6 +120,11 @@ int gbees_prune(gbees_ctx* ctx);
  * z [n], R [n*n row-major SPD]: host. Does not prune. */
 int gbees_correct(gbees_ctx* ctx, const double* z, const double* R);
 
+/* Eq. (4) with a linear measurement model y = H x + v, v ~ N(0, R) (the paper's own scenario measures
+ * one state only: y = x3): P_c <- P_c * exp(-1/2 (y - H x_c)^T R^-1 (y - H x_c)),
+ * renormalise. H [m*n row-major], y [m], R [m*m row-major SPD]: host; 1 <= m <= 6. Does not prune. */
+int gbees_correct_linear(gbees_ctx* ctx, const double* H, int m, const double* y, const double* R);
+
 /* Write the active cells in unspecified order: keys [cap*n] int32 row-major, p [cap] (normalised).
  * Buffers: host or device (detected), caller-owned. keys == NULL and p == NULL: only *count.
  * cap < count: nothing written, *count = needed, GBEES_ERR_BUFFER. count: host pointer. */

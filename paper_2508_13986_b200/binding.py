@@ -57,6 +57,7 @@ def lib():
         L.gbees_run.argtypes = [vp, C.c_double, C.c_int64, C.c_int, C.POINTER(C.c_int64)]
         L.gbees_count.argtypes = [vp, C.POINTER(C.c_int64)]
         L.gbees_time.argtypes = [vp, dp]
+        L.gbees_correct_linear.argtypes = [vp, dp, C.c_int, dp, dp]
         L.gbees_stats.argtypes = [vp, C.POINTER(Stats)]
         L.gbees_profile.argtypes = [vp, C.c_int, dp, C.POINTER(C.c_int64)]
         L.gbees_run_breakdown.argtypes = [vp, dp]
@@ -136,6 +137,12 @@ class Gbees:
         _, zp = _d(z)
         _, rp = _d(R)
         self._chk(lib().gbees_correct(self._h, zp, rp))
+
+    def correct_linear(self, H, y, R):
+        Ha, hp = _d(H)
+        ya, yp = _d(y)
+        _, rp = _d(R)
+        self._chk(lib().gbees_correct_linear(self._h, hp, int(ya.size), yp, rp))
 
     def run(self, t_target, max_steps=1 << 62, prune_every=0):
         done = C.c_int64()

@@ -193,6 +193,8 @@ __global__ void __launch_bounds__(TPB) k_init_gaussian(GP, const __grid_constant
 template <int NDIM>
 __global__ void __launch_bounds__(TPB) k_correct(GP, const __grid_constant__ GaussArgs g) { ST; phase_correct<NDIM>(p, st, ds, g); }
 template <int NDIM>
+__global__ void __launch_bounds__(TPB) k_correct_linear(GP, const __grid_constant__ GaussArgs g) { ST; phase_correct_linear<NDIM>(p, st, ds, g); }
+template <int NDIM>
 __global__ void __launch_bounds__(TPB) k_export(GP, int32_t* keys, double* out) { ST; phase_export<NDIM>(p, st, ds, keys, out); }
 template <int NDIM, bool FILL>
 __global__ void __launch_bounds__(TPB) k_import(GP, const int32_t* keys, const double* vals, uint64_t count) {
@@ -690,6 +692,29 @@ int gbees_correct(gbees_ctx* c, const double* z, const double* R) {
     phase(c, GBEES_PH_CORRECT, 3, [&] {
         dispatch_n(c, [&](auto N_) {
             k_correct<decltype(N_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, g);
+            return GBEES_OK;
+        });
+        k_sum<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 0, 0);
+        k_finish<<<1, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, c->grid, 1, 0);
+    });
+    CU(cudaGetLastError());
+    return sync_state(c);
+}
+
+int gbees_correct_linear(gbees_ctx* c, const double* H, int m, const double* y, const double* R) {
+    if (!c || !H || !y || !R || m < 1 || m > MAXN) return GBEES_ERR_ARG;
+    if (c->sticky) return c->sticky;
+    CU(cudaSetDevice(c->device));
+    GaussArgs g;
+    std::memset(&g, 0, sizeof(g));
+    double det;
+    if (!spd_inverse(m, R, g.inv, &det)) return GBEES_ERR_NOT_SPD;
+    g.m = m;
+    for (int k = 0; k < m * c->p.n; ++k) g.H[k] = H[k];
+    for (int r = 0; r < m; ++r) g.v[r] = y[r];
+    phase(c, GBEES_PH_CORRECT, 3, [&] {
+        dispatch_n(c, [&](auto N_) {
+            k_correct_linear<decltype(N_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, g);
             return GBEES_OK;
         });
         k_sum<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 0, 0);

@@ -734,7 +734,9 @@ __device__ inline void phase_rebuild(const Params& p, const Store& st, DevState*
 // ---- D5 / A8 init_gaussian: one thread per candidate cell of the ellipsoid's bounding box ---------
 struct GaussArgs {
     double inv[MAXN * MAXN];   // Sigma^-1 (or R^-1 for correct)
-    double v[MAXN];            // correct: measurement z
+    double H[MAXN * MAXN];     // correct_linear: measurement matrix, m x n row-major
+    int m;                     // correct_linear: number of measured quantities
+    double v[MAXN];            // correct: measurement z (or y)
     double norm;               // P~ at the mean
     int64_t R[MAXN];           // half-extents of the bounding box in cells
     unsigned long long total;  // prod (2 R_j + 1)
@@ -843,6 +845,42 @@ __device__ void phase_correct(const Params& p, const Store& st, DevState* ds, co
 #pragma unroll
         for (int j = 0; j < NDIM; ++j) d[j] = g.v[j] - (p.mu[j] + (double)c[j] * p.h[j]);
         st.Q[i] *= exp(-0.5 * quad_form<NDIM>(g.inv, d));
+    }
+}
+
+// f2, Eq. (4) with y = H x + v (the paper's scenario measures x3 only):
+// Q_c *= exp(-1/2 (y - H x_c)^T R^-1 (y - H x_c))
+template <int NDIM>
+__device__ void phase_correct_linear(const Params& p, const Store& st, DevState* ds, const GaussArgs& g) {
+    const uint32_t NB = min(ds->NB, p.capB);
+    const uint64_t items = (uint64_t)NB * 64;
+    const int m = g.m;
+    for (uint64_t i = gtid(); i < items; i += gthreads()) {
+        const uint32_t b = (uint32_t)(i >> 6);
+        const int l = (int)(i & 63);
+        if (!((st.mask[b] >> l) & 1ull)) continue;
+        int32_t B[NDIM], c[NDIM];
+        unpack<NDIM>(p, st.bkey[b], B);
+        cell_coords<NDIM>(B, l, c);
+        double x[NDIM], d[MAXN];
+#pragma unroll
+        for (int j = 0; j < NDIM; ++j) x[j] = p.mu[j] + (double)c[j] * p.h[j];
+#pragma unroll
+        for (int r = 0; r < MAXN; ++r) {
+            double hx = 0.0;
+#pragma unroll
+            for (int j = 0; j < NDIM; ++j) hx += g.H[r * NDIM + j] * x[j];
+            d[r] = r < m ? g.v[r] - hx : 0.0;
+        }
+        double q = 0.0;
+#pragma unroll
+        for (int r = 0; r < MAXN; ++r) {
+            double t = 0.0;
+#pragma unroll
+            for (int k = 0; k < MAXN; ++k) t += (r < m && k < m) ? g.inv[r * m + k] * d[k] : 0.0;
+            q += d[r] * t;
+        }
+        st.Q[i] *= exp(-0.5 * q);
     }
 }
 

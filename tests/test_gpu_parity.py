@@ -301,3 +301,48 @@ def test_export_buffer_contract_and_device_export():
     with pytest.raises(GbeesError) as e:
         g2.prune()
     assert e.value.code == -6
+
+
+def test_correct_linear_partial_state_parity():
+    """f2: Eq. (4) with y = H x + v on the GPU against the oracle (single-state and 2 x 3 measurement)."""
+    cfg = W.config0()
+    for H, y, R in [(np.array([[0.0, 0.0, 1.0]]), np.array([9.1]), np.array([[1.0]])),
+                    (np.array([[1.0, 0.0, 0.5], [0.0, 2.0, -1.0]]), np.array([-6.9, -29.2]), np.array([[0.9, 0.2], [0.2, 1.4]]))]:
+        g = G(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfg["cfl"], max_cells=cfg["max_cells"])
+        o = Oracle(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfg["cfl"])
+        g.init_gaussian(cfg["mean"], cfg["cov"]); o.init_gaussian(cfg["mean"], cfg["cov"])
+        for _ in range(3):
+            g.step(); o.step(); g.prune(); o.prune()
+        g.correct_linear(H, y, R); o.correct_linear(H, y, R)
+        compare_states(*g.export(), *o.export(), cfg["thresh"], 1e-10, what="after correct_linear")
+        g.prune(); o.prune()
+        g.step(); o.step()
+        compare_states(*g.export(), *o.export(), cfg["thresh"], 1e-10, what="correct_linear + prune + step")
+
+
+def test_paper_lorenz63_scenario_soft_sanity():
+    """The paper's own Lorenz '63 run: z-shifted form with (sigma, b, r) = (4, 1, 48),
+    h = 0.5, dt = 1.0 x CFL, t in [0, 2], one measurement y = x3 = -8 (sigma_y = 1) at t = 1. GPU == oracle
+    at 1e-8; SOFT comparison with Table 2 (~960 steps, ~24 k cells at most): the
+    paper's threshold is not stated, so only the order of magnitude is asserted."""
+    par, mean, dx, thr = [4.0, 1.0, 48.0], [-11.5, -10.0, 9.5], [0.5] * 3, 2e-5
+    g = G(3, dx, thr, W.DYN_L63_PAPER, par, cfl=1.0, max_cells=1 << 20)
+    o = Oracle(3, dx, thr, W.DYN_L63_PAPER, par, cfl=1.0)
+    g.init_gaussian(mean, np.eye(3)); o.init_gaussian(mean, np.eye(3))
+    steps, max_cells = 0, o.count()
+    for leg, t_end in enumerate([1.0, 2.0]):
+        k = 0
+        while o.time() < t_end:
+            o.step(t_end - o.time()); o.prune(); k += 1
+            max_cells = max(max_cells, o.count())
+        assert g.run(t_end, prune_every=1) == k
+        steps += k
+        assert g.time() == o.time() == t_end
+        compare_states(*g.export(), *o.export(), thr, 1e-8, what=f"paper L63 scenario, t = {t_end}")
+        if leg == 0:
+            H, y, R = np.array([[0.0, 0.0, 1.0]]), np.array([-8.0]), np.array([[1.0]])
+            g.correct_linear(H, y, R); o.correct_linear(H, y, R)
+            g.prune(); o.prune()
+            compare_states(*g.export(), *o.export(), thr, 1e-8, what="after the measurement at t = 1")
+    print(f"paper L63 scenario: {steps} steps (paper ~960), max {max_cells} cells (paper ~24 k)")
+    assert 300 <= steps <= 3000 and 2_000 <= max_cells <= 240_000
