@@ -445,3 +445,24 @@ def test_P13_reflection(axis):
     d2 = as_dict(k2 * M.diagonal().astype(np.int32), p2)
     assert d1.keys() == d2.keys()
     assert max(abs(d1[k] - d2[k]) for k in d1) <= 1e-14 * p1.max()
+
+
+def test_F1_metrics_oracle_pins():
+    """BC (Eq. 9) and the 1-norm E: identical -> (1, 0), disjoint -> (0, 2), and two
+    discretised 1-D Gaussians N(0, s^2), N(d, s^2): BC -> exp(-d^2 / (8 s^2)), E -> 2 (2 Phi(d / 2s) - 1)."""
+    from math import erf, exp, sqrt
+    from oracle import metrics_oracle as M
+    h, s, d = 0.01, 1.0, 0.7
+    k = np.arange(-900, 1000)[:, None]
+    x = k[:, 0] * h
+    pa = np.exp(-0.5 * (x / s) ** 2); pa /= pa.sum()
+    pb = np.exp(-0.5 * ((x - d) / s) ** 2); pb /= pb.sum()
+    assert M.bc_and_l1(k, pa, k, pa) == (pytest.approx(1.0, abs=1e-12), 0.0)
+    assert M.bc_and_l1(k, pa, k + 5000, pa) == (0.0, pytest.approx(2.0, abs=1e-12))
+    bc, l1 = M.bc_and_l1(k, pa, k, pb)
+    assert bc == pytest.approx(exp(-d * d / (8 * s * s)), abs=1e-6)
+    assert l1 == pytest.approx(2 * (2 * 0.5 * (1 + erf(d / (2 * s) / sqrt(2))) - 1), abs=1e-4)
+    # partially overlapping key sets: cells present on one side only count with probability 0 on the other
+    ka, kb = np.array([[0], [1], [2]]), np.array([[1], [2], [3]])
+    bc, l1 = M.bc_and_l1(ka, np.array([0.5, 0.25, 0.25]), kb, np.array([0.25, 0.25, 0.5]))
+    assert bc == pytest.approx(sqrt(0.25 * 0.25) + 0.25) and l1 == pytest.approx(0.5 + 0.0 + 0.0 + 0.5)
