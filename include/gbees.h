@@ -125,6 +125,12 @@ int gbees_correct(gbees_ctx* ctx, const double* z, const double* R);
  * renormalise. H [m*n row-major], y [m], R [m*m row-major SPD]: host; 1 <= m <= 6. Does not prune. */
 int gbees_correct_linear(gbees_ctx* ctx, const double* H, int m, const double* y, const double* R);
 
+/* Distribution metrics between two contexts on the SAME grid (same n, dx, origin, device; else
+ * GBEES_ERR_ARG): *bc = sum_c sqrt(Pa_c Pb_c) (Bhattacharyya coefficient, Eq. 9) and
+ * *l1 = sum_c |Pa_c - Pb_c| (the paper's 1-norm E of PAPER.md:362-366 in cell masses), over the union
+ * of the two active sets. bc, l1: host. Neither context is modified. */
+int gbees_compare(gbees_ctx* ctx, gbees_ctx* other, double* bc, double* l1);
+
 /* Write the active cells in unspecified order: keys [cap*n] int32 row-major, p [cap] (normalised).
  * Buffers: host or device (detected), caller-owned. keys == NULL and p == NULL: only *count.
  * cap < count: nothing written, *count = needed, GBEES_ERR_BUFFER. count: host pointer. */

@@ -58,6 +58,7 @@ def lib():
         L.gbees_count.argtypes = [vp, C.POINTER(C.c_int64)]
         L.gbees_time.argtypes = [vp, dp]
         L.gbees_correct_linear.argtypes = [vp, dp, C.c_int, dp, dp]
+        L.gbees_compare.argtypes = [vp, vp, dp, dp]
         L.gbees_stats.argtypes = [vp, C.POINTER(Stats)]
         L.gbees_profile.argtypes = [vp, C.c_int, dp, C.POINTER(C.c_int64)]
         L.gbees_run_breakdown.argtypes = [vp, dp]
@@ -143,6 +144,12 @@ class Gbees:
         ya, yp = _d(y)
         _, rp = _d(R)
         self._chk(lib().gbees_correct_linear(self._h, hp, int(ya.size), yp, rp))
+
+    def compare(self, other):
+        """(BC, E) between this context and another one on the same grid (Eq. 9 and the 1-norm of PAPER.md:362-366)."""
+        bc, l1 = C.c_double(), C.c_double()
+        self._chk(lib().gbees_compare(self._h, other._h, C.byref(bc), C.byref(l1)))
+        return bc.value, l1.value
 
     def run(self, t_target, max_steps=1 << 62, prune_every=0):
         done = C.c_int64()

@@ -195,6 +195,21 @@ __global__ void __launch_bounds__(TPB) k_correct(GP, const __grid_constant__ Gau
 template <int NDIM>
 __global__ void __launch_bounds__(TPB) k_correct_linear(GP, const __grid_constant__ GaussArgs g) { ST; phase_correct_linear<NDIM>(p, st, ds, g); }
 template <int NDIM>
+__global__ void __launch_bounds__(TPB) k_compare(const __grid_constant__ Params p, const __grid_constant__ Store a_in, const DevState* da,
+                                                 const __grid_constant__ Store b_in, const DevState* db, double* out) {
+    const Store a = resolve(a_in, da), b = resolve(b_in, db);
+    phase_compare<NDIM>(p, a, da, b, db, out);
+}
+// sums the three rows of per-block partials in index order: out3[0..2]
+__global__ void __launch_bounds__(TPB) k_compare_finish(const double* part, unsigned nparts, double* out3) {
+    for (int q = 0; q < 3; ++q) {
+        double v = 0.0;
+        for (unsigned k = threadIdx.x; k < nparts; k += blockDim.x) v += part[(size_t)q * nparts + k];
+        v = block_sum(v);
+        if (threadIdx.x == 0) out3[q] = v;
+    }
+}
+template <int NDIM>
 __global__ void __launch_bounds__(TPB) k_export(GP, int32_t* keys, double* out) { ST; phase_export<NDIM>(p, st, ds, keys, out); }
 template <int NDIM, bool FILL>
 __global__ void __launch_bounds__(TPB) k_import(GP, const int32_t* keys, const double* vals, uint64_t count) {
@@ -722,6 +737,35 @@ int gbees_correct_linear(gbees_ctx* c, const double* H, int m, const double* y, 
     });
     CU(cudaGetLastError());
     return sync_state(c);
+}
+
+int gbees_compare(gbees_ctx* c, gbees_ctx* o, double* bc, double* l1) {
+    if (!c || !o || !bc || !l1) return GBEES_ERR_ARG;
+    if (c->sticky) return c->sticky;
+    if (o->sticky) return o->sticky;
+    if (c->p.n != o->p.n || c->device != o->device) return GBEES_ERR_ARG;
+    for (int j = 0; j < c->p.n; ++j)
+        if (c->p.h[j] != o->p.h[j] || c->p.mu[j] != o->p.mu[j]) return GBEES_ERR_ARG;   // same grid only
+    CU(cudaSetDevice(c->device));
+    CU(cudaStreamSynchronize(o->stream));            // the other context's state is complete
+    CU(cudaStreamSynchronize(c->stream));
+    double* part = c->st.phi;                          // free between steps: 3 x grid partials + 2 x 3 results
+    double* res = part + 3 * (size_t)c->grid;
+    dispatch_n(c, [&](auto N_) {
+        k_compare<decltype(N_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, o->st, o->d_st, part);
+        k_compare_finish<<<1, TPB, 0, c->stream>>>(part, c->grid, res);
+        k_compare<decltype(N_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, o->st, o->d_st, c->st, c->d_st, part);
+        k_compare_finish<<<1, TPB, 0, c->stream>>>(part, c->grid, res + 3);
+        return GBEES_OK;
+    });
+    c->launches += 4;
+    CU(cudaGetLastError());
+    double h[6];
+    CU(cudaMemcpyAsync(h, res, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    *bc = h[0];
+    *l1 = h[1] + h[5];     // |Pa - Pb| over this grid's cells + |Pb| over the cells only the other grid has
+    return GBEES_OK;
 }
 
 int gbees_export(gbees_ctx* c, int32_t* keys, double* pv, int64_t cap, int64_t* count) {

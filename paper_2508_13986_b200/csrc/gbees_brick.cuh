@@ -884,6 +884,41 @@ __device__ void phase_correct_linear(const Params& p, const Store& st, DevState*
     }
 }
 
+// f1, distribution metrics between two contexts on the same grid (same n, dx, origin):
+//   BC = sum_c sqrt(Pa_c Pb_c)  (Eq. 9),  E = sum_c |Pa_c - Pb_c|  (masses).
+// One warp per brick of A looks the brick up in B's table (hash join over BRICK keys); per-block
+// partials of (BC, sum |Pa - Pb| over A's cells, sum |Pa| over A's cells that B does not have) go to
+// out[3][gridDim.x]. The host runs it both ways: E = (second sum of A->B) + (third sum of B->A).
+template <int NDIM>
+__device__ void phase_compare(const Params& p, const Store& a, const DevState* da, const Store& b, const DevState* db,
+                              double* out) {
+    const uint32_t NBa = min(da->NB, p.capB);
+    const double sa = da->scale, sb = db->scale;
+    const uint64_t slots_b = db->slots;
+    const unsigned lane = lane_id();
+    double bc = 0.0, l1 = 0.0, mb = 0.0;
+    for (uint32_t r = gwarp(); r < NBa; r += gwarps()) {
+        const uint64_t ma = a.mask[r];
+        if (!ma) continue;
+        const uint32_t rb = ht_find(b.table, slots_b, a.bkey[r]);
+        const uint64_t mbk = rb != NBR_NONE ? b.mask[rb] : 0ull;
+#pragma unroll
+        for (int hh = 0; hh < 2; ++hh) {
+            const int l = (int)lane + 32 * hh;
+            if (!((ma >> l) & 1ull)) continue;
+            const double pa = sa * a.Q[(size_t)r * 64 + l];
+            const double pb = ((mbk >> l) & 1ull) ? sb * b.Q[(size_t)rb * 64 + l] : 0.0;
+            if (pa > 0.0 && pb > 0.0) bc += sqrt(pa * pb);
+            l1 += fabs(pa - pb);
+            if (!((mbk >> l) & 1ull)) mb += fabs(pa);
+        }
+    }
+    bc = block_sum(bc);
+    l1 = block_sum(l1);
+    mb = block_sum(mb);
+    if (threadIdx.x == 0) { out[blockIdx.x] = bc; out[gridDim.x + blockIdx.x] = l1; out[2 * gridDim.x + blockIdx.x] = mb; }
+}
+
 // export: a warp reserves popc(mask) output rows per brick (order of bricks is unspecified)
 template <int NDIM>
 __device__ void phase_export(const Params& p, const Store& st, DevState* ds, int32_t* keys, double* out) {

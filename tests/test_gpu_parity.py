@@ -346,3 +346,36 @@ def test_paper_lorenz63_scenario_soft_sanity():
             compare_states(*g.export(), *o.export(), thr, 1e-8, what="after the measurement at t = 1")
     print(f"paper L63 scenario: {steps} steps (paper ~960), max {max_cells} cells (paper ~24 k)")
     assert 300 <= steps <= 3000 and 2_000 <= max_cells <= 240_000
+
+
+def test_compare_metrics_and_temporal_convergence():
+    """f1: BC (Eq. 9) and the 1-norm E between two GPU runs on the same grid, checked
+    against the metrics oracle applied to the exported states; and the paper's temporal-convergence
+    protocol: E against a reference run with a very small epsilon decreases with epsilon."""
+    from oracle import metrics_oracle as M
+    cfg = W.config0()
+
+    def run(cfl):
+        g = G(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfl, max_cells=1 << 18)
+        g.init_gaussian(cfg["mean"], cfg["cov"])
+        g.run(0.05, prune_every=1)
+        assert g.time() == 0.05
+        return g
+
+    ref = run(0.02)
+    rk, rp = ref.export()
+    errs = []
+    for eps in (1.0, 0.5, 0.2):
+        g = run(eps)
+        bc, l1 = g.compare(ref)
+        obc, ol1 = M.bc_and_l1(*g.export(), rk, rp)
+        assert bc == pytest.approx(obc, rel=1e-12) and l1 == pytest.approx(ol1, rel=1e-10, abs=1e-13)
+        bc2, l12 = ref.compare(g)                                   # symmetric
+        assert bc2 == pytest.approx(bc, rel=1e-12) and l12 == pytest.approx(l1, rel=1e-10, abs=1e-13)
+        assert 0.9 < bc <= 1.0 + 1e-4
+        errs.append(l1)
+    assert errs[0] > errs[1] > errs[2] > 0.0
+    # a run against itself: E = 0; BC = sum of the positive masses = 1 + |negative mass| (A5: negatives are kept)
+    bc, l1 = ref.compare(ref)
+    assert l1 == 0.0 and bc == pytest.approx(rp[rp > 0].sum(), rel=1e-12) and abs(bc - 1.0) < 1e-4
+    print("temporal convergence, E(eps = 1, 0.5, 0.2) vs eps = 0.02:", errs)
