@@ -466,3 +466,21 @@ def test_F1_metrics_oracle_pins():
     ka, kb = np.array([[0], [1], [2]]), np.array([[1], [2], [3]])
     bc, l1 = M.bc_and_l1(ka, np.array([0.5, 0.25, 0.25]), kb, np.array([0.25, 0.25, 0.5]))
     assert bc == pytest.approx(sqrt(0.25 * 0.25) + 0.25) and l1 == pytest.approx(0.5 + 0.0 + 0.0 + 0.5)
+
+
+def test_F3_marginal_oracle_pins():
+    """Marginals: mass is preserved, the marginal of a product measure is its factor,
+    and integrating out nothing / everything gives the PDF itself / the total mass."""
+    from oracle import marginal_oracle as MO
+    rng = np.random.default_rng(5)
+    a, b, c = rng.random(5), rng.random(4), rng.random(3)
+    keys = np.array([[i, j, k] for i in range(5) for j in range(4) for k in range(3)], dtype=np.int32) - 2
+    p = np.array([a[i] * b[j] * c[k] for i in range(5) for j in range(4) for k in range(3)])
+    k1, m1 = MO.marginal(keys, p, [1])
+    assert np.array_equal(k1[:, 0], np.arange(4) - 2) and np.allclose(m1, b * a.sum() * c.sum(), rtol=1e-14)
+    k02, m02 = MO.marginal(keys, p, [2, 0])                 # kept dims in the order asked for
+    want = {(k - 2, i - 2): c[k] * a[i] * b.sum() for i in range(5) for k in range(3)}
+    assert all(abs(want[tuple(kk)] - v) < 1e-14 for kk, v in zip(k02.tolist(), m02.tolist())) and len(k02) == 15
+    assert m02.sum() == pytest.approx(p.sum(), rel=1e-14)
+    kall, mall = MO.marginal(keys, p, [0, 1, 2])
+    assert np.array_equal(kall, keys) and np.array_equal(mall, p)
