@@ -131,6 +131,13 @@ int gbees_correct_linear(gbees_ctx* ctx, const double* H, int m, const double* y
  * of the two active sets. bc, l1: host. Neither context is modified. */
 int gbees_compare(gbees_ctx* ctx, gbees_ctx* other, double* bc, double* l1);
 
+/* Marginal PDF: sum the cell probabilities over the dimensions NOT listed in
+ * dims [m] (host; distinct indices in [0, n), output order = order in dims), hash-accumulated on the
+ * device. Writes *count marginal cells in unspecified order: keys [cap*m] int32 row-major, p [cap]
+ * (host or device buffers, caller-owned); keys == NULL or p == NULL: only *count; cap < *count:
+ * GBEES_ERR_BUFFER. The additions are atomic, so the last bits of p may differ between calls. */
+int gbees_marginal(gbees_ctx* ctx, const int* dims, int m, int32_t* keys, double* p, int64_t cap, int64_t* count);
+
 /* Write the active cells in unspecified order: keys [cap*n] int32 row-major, p [cap] (normalised).
  * Buffers: host or device (detected), caller-owned. keys == NULL and p == NULL: only *count.
  * cap < count: nothing written, *count = needed, GBEES_ERR_BUFFER. count: host pointer. */

@@ -59,6 +59,7 @@ def lib():
         L.gbees_time.argtypes = [vp, dp]
         L.gbees_correct_linear.argtypes = [vp, dp, C.c_int, dp, dp]
         L.gbees_compare.argtypes = [vp, vp, dp, dp]
+        L.gbees_marginal.argtypes = [vp, C.POINTER(C.c_int), C.c_int, vp, vp, C.c_int64, C.POINTER(C.c_int64)]
         L.gbees_stats.argtypes = [vp, C.POINTER(Stats)]
         L.gbees_profile.argtypes = [vp, C.c_int, dp, C.POINTER(C.c_int64)]
         L.gbees_run_breakdown.argtypes = [vp, dp]
@@ -150,6 +151,20 @@ class Gbees:
         bc, l1 = C.c_double(), C.c_double()
         self._chk(lib().gbees_compare(self._h, other._h, C.byref(bc), C.byref(l1)))
         return bc.value, l1.value
+
+    def marginal(self, dims, sort=True):
+        """Host marginal over the kept dimensions `dims`: (keys int32 [M, m], p float64 [M])."""
+        d = (C.c_int * len(dims))(*[int(x) for x in dims])
+        cnt = C.c_int64()
+        self._chk(lib().gbees_marginal(self._h, d, len(dims), None, None, 0, C.byref(cnt)))
+        M = cnt.value
+        keys = np.empty((M, len(dims)), dtype=np.int32)
+        p = np.empty(M, dtype=np.float64)
+        self._chk(lib().gbees_marginal(self._h, d, len(dims), keys.ctypes.data, p.ctypes.data, M, C.byref(cnt)))
+        if sort and M:
+            order = np.lexsort(keys.T[::-1])
+            keys, p = keys[order], p[order]
+        return keys, p
 
     def run(self, t_target, max_steps=1 << 62, prune_every=0):
         done = C.c_int64()

@@ -209,6 +209,16 @@ __global__ void __launch_bounds__(TPB) k_compare_finish(const double* part, unsi
         if (threadIdx.x == 0) out3[q] = v;
     }
 }
+__global__ void __launch_bounds__(TPB) k_marg_clear(unsigned long long* skey, double* sval, unsigned long long S) { phase_marg_clear(skey, sval, S); }
+template <int NDIM>
+__global__ void __launch_bounds__(TPB) k_marg_accumulate(GP, const __grid_constant__ MargArgs g, unsigned long long* skey, double* sval) {
+    ST;
+    phase_marg_accumulate<NDIM>(p, st, ds, g, skey, sval);
+}
+__global__ void __launch_bounds__(TPB) k_marg_emit(DevState* ds, const __grid_constant__ MargArgs g, const unsigned long long* skey,
+                                                   const double* sval, int32_t* keys, double* out, unsigned cap) {
+    phase_marg_emit(ds, g, skey, sval, keys, out, cap);
+}
 template <int NDIM>
 __global__ void __launch_bounds__(TPB) k_export(GP, int32_t* keys, double* out) { ST; phase_export<NDIM>(p, st, ds, keys, out); }
 template <int NDIM, bool FILL>
@@ -765,6 +775,63 @@ int gbees_compare(gbees_ctx* c, gbees_ctx* o, double* bc, double* l1) {
     CU(cudaStreamSynchronize(c->stream));
     *bc = h[0];
     *l1 = h[1] + h[5];     // |Pa - Pb| over this grid's cells + |Pb| over the cells only the other grid has
+    return GBEES_OK;
+}
+
+int gbees_marginal(gbees_ctx* c, const int* dims, int m, int32_t* keys, double* pv, int64_t cap, int64_t* count) {
+    if (!c || !dims || !count || m < 1 || m > c->p.n) return GBEES_ERR_ARG;
+    if (c->sticky) return c->sticky;
+    MargArgs g;
+    std::memset(&g, 0, sizeof(g));
+    g.m = m;
+    for (int r = 0; r < m; ++r) {
+        if (dims[r] < 0 || dims[r] >= c->p.n) return GBEES_ERR_ARG;
+        for (int q = 0; q < r; ++q) if (dims[q] == dims[r]) return GBEES_ERR_ARG;
+        g.dims[r] = dims[r];
+    }
+    g.mbits = 63 / m > 32 ? 32 : 63 / m;
+    if (g.mbits < c->p.bits) g.mbits = c->p.bits;                 // m <= n, so floor(63/m) >= floor(63/n) anyway
+    const unsigned long long N = c->h_st->N;
+    if (N == 0) { *count = 0; return GBEES_OK; }
+    CU(cudaSetDevice(c->device));
+    g.S = 1024;
+    while (g.S < 2 * N) g.S <<= 1;                                // at most N marginal cells: load factor <= 0.5
+    // scratch in the phi array (free between steps): table keys, table values, then the output staging area
+    const size_t need = (size_t)g.S * 16 + (size_t)N * (4 * (size_t)m + 8) + 64;
+    if (need > c->stage_bytes) return fail(c, GBEES_ERR_CAPACITY, "marginal: scratch larger than the staging area");
+    unsigned long long* skey = reinterpret_cast<unsigned long long*>(c->st.phi);
+    double* sval = reinterpret_cast<double*>(skey + g.S);
+    char* stage = reinterpret_cast<char*>(sval + g.S);
+    auto on_device = [](const void* ptr) {
+        cudaPointerAttributes a;
+        if (cudaPointerGetAttributes(&a, ptr) != cudaSuccess) { cudaGetLastError(); return false; }
+        return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+    };
+    const bool dev_out = keys && pv && on_device(keys) && on_device(pv);
+    const unsigned ucap = keys && pv ? (dev_out ? (unsigned)(cap < (int64_t)N ? cap : (int64_t)N) : (unsigned)N) : 0u;
+    const size_t kbytes = ((size_t)N * m * 4 + 7) & ~(size_t)7;
+    int32_t* dk = dev_out ? keys : reinterpret_cast<int32_t*>(stage);
+    double* dp = dev_out ? pv : reinterpret_cast<double*>(stage + kbytes);
+    CU(cudaMemsetAsync(&c->d_st->export_count, 0, sizeof(unsigned), c->stream));
+    k_marg_clear<<<c->grid, TPB, 0, c->stream>>>(skey, sval, g.S);
+    dispatch_n(c, [&](auto N_) {
+        k_marg_accumulate<decltype(N_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, g, skey, sval);
+        return GBEES_OK;
+    });
+    k_marg_emit<<<c->grid, TPB, 0, c->stream>>>(c->d_st, g, skey, sval, dk, dp, ucap);
+    c->launches += 3;
+    CU(cudaGetLastError());
+    unsigned got = 0;
+    CU(cudaMemcpyAsync(&got, &c->d_st->export_count, sizeof(unsigned), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    *count = got;
+    if (!keys || !pv) return GBEES_OK;                            // count only
+    if (cap < (int64_t)got) return GBEES_ERR_BUFFER;
+    if (!dev_out) {
+        CU(cudaMemcpyAsync(keys, dk, (size_t)got * m * 4, cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaMemcpyAsync(pv, dp, (size_t)got * 8, cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+    }
     return GBEES_OK;
 }
 

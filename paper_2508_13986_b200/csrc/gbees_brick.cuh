@@ -919,6 +919,65 @@ __device__ void phase_compare(const Params& p, const Store& a, const DevState* d
     if (threadIdx.x == 0) { out[blockIdx.x] = bc; out[gridDim.x + blockIdx.x] = l1; out[2 * gridDim.x + blockIdx.x] = mb; }
 }
 
+// f3, marginal PDF: the masses are hash-accumulated over the kept coordinates.
+// Scratch table: skey[S] (packed kept coordinates, KEY_EMPTY = free) and sval[S] (mass), linear probing
+// with the same mixer as the brick table; atomicAdd(double) accumulates, so the order of the additions
+// is not fixed (rounding-level differences between runs, as the paper notes for CUDA).
+struct MargArgs {
+    int m;                 // kept dimensions
+    int dims[MAXN];        // their indices, in output order
+    int mbits;             // bits per kept coordinate in the scratch key
+    unsigned long long S;  // scratch slots
+};
+__device__ __forceinline__ void phase_marg_clear(unsigned long long* skey, double* sval, unsigned long long S) {
+    for (unsigned long long i = gtid(); i < S; i += gthreads()) { skey[i] = KEY_EMPTY; sval[i] = 0.0; }
+}
+template <int NDIM>
+__device__ void phase_marg_accumulate(const Params& p, const Store& st, DevState* ds, const MargArgs& g,
+                                      unsigned long long* skey, double* sval) {
+    const uint32_t NB = min(ds->NB, p.capB);
+    const uint64_t items = (uint64_t)NB * 64;
+    const double scale = ds->scale;
+    const long long mbias = 1ll << (g.mbits - 1);
+    for (uint64_t i = gtid(); i < items; i += gthreads()) {
+        const uint32_t b = (uint32_t)(i >> 6);
+        const int l = (int)(i & 63);
+        if (!((st.mask[b] >> l) & 1ull)) continue;
+        int32_t B[NDIM], c[NDIM];
+        unpack<NDIM>(p, st.bkey[b], B);
+        cell_coords<NDIM>(B, l, c);
+        unsigned long long key = 0ull;
+        for (int r = 0; r < g.m; ++r) {
+            int32_t cv = 0;
+#pragma unroll
+            for (int j = 0; j < NDIM; ++j) if (g.dims[r] == j) cv = c[j];
+            key = (key << g.mbits) | (unsigned long long)((long long)cv + mbias);
+        }
+        unsigned long long s = home_slot(key, g.S);
+        for (;;) {
+            unsigned long long cur = *reinterpret_cast<volatile unsigned long long*>(&skey[s]);
+            if (cur == KEY_EMPTY) cur = atomicCAS(&skey[s], KEY_EMPTY, key);
+            if (cur == KEY_EMPTY || cur == key) break;
+            if (++s == g.S) s = 0;
+        }
+        atomicAdd(&sval[s], scale * st.Q[i]);
+    }
+}
+__device__ __forceinline__ void phase_marg_emit(DevState* ds, const MargArgs& g, const unsigned long long* skey,
+                                                const double* sval, int32_t* keys, double* out, unsigned cap) {
+    const long long mbias = 1ll << (g.mbits - 1);
+    const unsigned long long fm = (1ull << g.mbits) - 1ull;
+    for (unsigned long long i = gtid(); i < g.S; i += gthreads()) {
+        const unsigned long long key = skey[i];
+        if (key == KEY_EMPTY) continue;
+        const unsigned o = atomicAdd(&ds->export_count, 1u);
+        if (o >= cap) continue;
+        for (int r = 0; r < g.m; ++r)
+            keys[(size_t)o * g.m + r] = (int32_t)((long long)((key >> ((g.m - 1 - r) * g.mbits)) & fm) - mbias);
+        out[o] = sval[i];
+    }
+}
+
 // export: a warp reserves popc(mask) output rows per brick (order of bricks is unspecified)
 template <int NDIM>
 __device__ void phase_export(const Params& p, const Store& st, DevState* ds, int32_t* keys, double* out) {

@@ -379,3 +379,31 @@ def test_compare_metrics_and_temporal_convergence():
     bc, l1 = ref.compare(ref)
     assert l1 == 0.0 and bc == pytest.approx(rp[rp > 0].sum(), rel=1e-12) and abs(bc - 1.0) < 1e-4
     print("temporal convergence, E(eps = 1, 0.5, 0.2) vs eps = 0.02:", errs)
+
+
+def test_marginals_of_the_6d_pdf():
+    """f3: the two 3-D marginals of the 6-D Lorenz '96 PDF (and a 1-D, a 2-D one with
+    permuted dimensions) by device hash-accumulation against the numpy group-by of the exported state."""
+    import ctypes as C
+    from oracle import marginal_oracle as MO
+    from paper_2508_13986_b200.binding import lib
+    cfg = W.config2()
+    cfg.update(thresh=1e-5, max_cells=1 << 20)
+    g = G(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfg["cfl"], max_cells=cfg["max_cells"])
+    g.init_gaussian(cfg["mean"], cfg["cov"])
+    g.run(1e300, max_steps=6, prune_every=5)
+    keys, p = g.export()
+    for dims in ([0, 1, 2], [3, 4, 5], [4], [5, 0], [0, 1, 2, 3, 4, 5]):
+        mk, mp = g.marginal(dims)
+        ok, op = MO.marginal(keys, p, dims)
+        assert np.array_equal(mk, ok), dims
+        assert np.max(np.abs(mp - op)) <= 1e-12 * op.max()
+        assert mp.sum() == pytest.approx(1.0, abs=1e-12)
+    # buffer contract: count only, too small a buffer
+    d = (C.c_int * 3)(0, 1, 2)
+    cnt = C.c_int64()
+    assert lib().gbees_marginal(g._h, d, 3, None, None, 0, C.byref(cnt)) == 0 and cnt.value == len(MO.marginal(keys, p, [0, 1, 2])[1])
+    small = np.empty((4, 3), dtype=np.int32); sp = np.empty(4)
+    assert lib().gbees_marginal(g._h, d, 3, small.ctypes.data, sp.ctypes.data, 4, C.byref(cnt)) == -5
+    bad = (C.c_int * 2)(1, 1)
+    assert lib().gbees_marginal(g._h, bad, 2, None, None, 0, C.byref(cnt)) == -1
