@@ -396,12 +396,12 @@ __device__ void phase_smax(const Params& p, const Store& st, DevState* ds) {
 // Shared memory of one warp in pass 1: the brick's own row and its 2n neighbour rows (values and
 // activity flags), the update accumulator, the per-cell fetch flags and the list of active slots.
 template <int NDIM>
-struct Flux1Smem {
+struct alignas(16) Flux1Smem {
     static constexpr int ROWS = 2 * NDIM + 1, OWN = 2 * NDIM;
-    double R[ROWS][64];
+    double R[ROWS][64];              // staged rows: 2n neighbour bricks, then the brick itself
     double acc[64];
+    unsigned long long M[ROWS];      // active masks of the staged rows
     uint16_t fl[64];
-    uint8_t A[ROWS][64];
     uint8_t list[64];
 };
 
@@ -422,27 +422,25 @@ __device__ void phase_flux1(const Params& p, const Store& st, DevState* ds) {
 #pragma unroll
     for (int j = 0; j < NDIM; ++j) tau[j] = dt / p.h[j];
     for (uint32_t b = gwarp(); b < NB; b += gwarps()) {   // warp-uniform
-        // ---- stage the 2n+1 rows (coalesced 256-byte loads) and their activity flags
+        // ---- stage the 2n+1 rows (LDGSTS: 16 bytes per lane = one 512-byte row per warp instruction,
+        // no register round trip); rows of missing neighbour bricks are zero-filled; masks go to sm.M.
+        // (One 512-byte TMA bulk copy per row was measured too: equal on cfg2, 1.6x slower on cfg3s.)
         uint32_t my_row = NBR_NONE;
         uint64_t my_mask = 0ull;
         if (lane < ND) my_row = st.adj[(size_t)b * ND + lane];
         if (lane == OWN) my_row = b;
         if (my_row != NBR_NONE) my_mask = st.mask[my_row];
         const uint64_t bk = st.bkey[b];
-        uint64_t m = 0ull;
+        if (lane < SM::ROWS) sm.M[lane] = my_mask;
 #pragma unroll
         for (int r = 0; r < SM::ROWS; ++r) {
             const uint32_t row = __shfl_sync(0xffffffffu, my_row, r);
-            const uint32_t mlo = __shfl_sync(0xffffffffu, (uint32_t)my_mask, r);
-            const uint32_t mhi = __shfl_sync(0xffffffffu, (uint32_t)(my_mask >> 32), r);
-            // global -> shared without a register round trip (LDGSTS, 16 bytes per lane = one row)
             if (row != NBR_NONE) __pipeline_memcpy_async(&sm.R[r][2 * lane], &Q[(size_t)row * 64 + 2 * lane], 16);
             else *reinterpret_cast<double2*>(&sm.R[r][2 * lane]) = make_double2(0.0, 0.0);
-            sm.A[r][lane] = (uint8_t)((mlo >> lane) & 1u);
-            sm.A[r][lane + 32] = (uint8_t)((mhi >> lane) & 1u);
-            if (r == OWN) m = ((uint64_t)mhi << 32) | mlo;
         }
         __pipeline_commit();
+        const uint64_t m = ((uint64_t)__shfl_sync(0xffffffffu, (uint32_t)(my_mask >> 32), OWN) << 32) |
+                           __shfl_sync(0xffffffffu, (uint32_t)my_mask, OWN);
         sm.acc[lane] = 0.0; sm.acc[lane + 32] = 0.0;
         sm.fl[lane] = 0; sm.fl[lane + 32] = 0;
         const uint32_t m_lo = (uint32_t)m, m_hi = (uint32_t)(m >> 32);
@@ -455,7 +453,7 @@ __device__ void phase_flux1(const Params& p, const Store& st, DevState* ds) {
         __pipeline_wait_prior(0);
         __syncwarp();
         const double* Rf = &sm.R[0][0];
-        const uint8_t* Af = &sm.A[0][0];
+        const unsigned long long* Mf = &sm.M[0];
         for (int r0 = 0; r0 < cnt; r0 += 32) {             // active cells, 32 at a time
             const bool act = r0 + (int)lane < cnt;
             const int l = act ? sm.list[r0 + lane] : 0;
@@ -476,8 +474,8 @@ __device__ void phase_flux1(const Params& p, const Store& st, DevState* ds) {
                     const int im = lj > 0 ? OWN * 64 + l - s : (2 * j) * 64 + l + MK * s;
                     const int ip = lj < MK ? OWN * 64 + l + s : (2 * j + 1) * 64 + l - MK * s;
                     const double vm = Rf[im], vp = Rf[ip];
-                    am |= (unsigned)Af[im] << j;
-                    ap |= (unsigned)Af[ip] << j;
+                    am |= (unsigned)((Mf[im >> 6] >> (im & 63)) & 1ull) << j;
+                    ap |= (unsigned)((Mf[ip >> 6] >> (ip & 63)) & 1ull) << j;
                     dm[j] = q0 - vm;
                     dp[j] = vp - q0;
                     double t = 0.0;
