@@ -132,6 +132,8 @@ __device__ void phase_targets(const Params& p, const Store& st, DevState* ds) {
     __shared__ unsigned long long sO[WPB][ND];        // O_d: sources with outflow through face d
     __shared__ unsigned long long sDiag[WPB][NT - ND > 0 ? NT - ND : 1];   // target bits bound for diagonal bricks, per edge class
     __shared__ uint32_t sAdj[WPB][ND];
+    __shared__ unsigned long long sTb[WPB][ND + 1];   // merged target bits per destination (face neighbours, own)
+    __shared__ uint8_t sItem[WPB][NT + 1];            // work list of the non-empty destinations / diagonal classes
     __shared__ unsigned long long sEdge[ND];
     __shared__ unsigned long long sQk[GROW ? WPB : 1][GROW ? NT : 1], sQm[GROW ? WPB : 1][GROW ? NT : 1];   // new cells: (brick key, bits)
     __shared__ unsigned sQn[WPB];
@@ -242,43 +244,58 @@ __device__ void phase_targets(const Params& p, const Store& st, DevState* ds) {
             }
         }
         __syncwarp();
-        // ---- apply: lane d <= 2n takes destination d; then the diagonal parts, one lane per class
-        if (lane <= ND && myT) {
-            const uint32_t row = lane == OWN ? b : sAdj[w][lane];
-            if (GROW) {
-                uint64_t key = bk;
-                if (lane != OWN) {
-                    const uint64_t u1 = 1ull << ((NDIM - 1 - (int)(lane >> 1)) * p.bits);
-                    key = (lane & 1) ? bk + u1 : bk - u1;
-                }
-                account(key, grow_apply(p, st, ds, NB0, slots, ND, row, key, myT));
-            } else if (row != NBR_NONE) {
-                const unsigned long long x = myT & st.mask[row];
-                if (x) atomicOr((unsigned long long*)&st.keep[row], x);
+        // ---- apply: the non-empty parts (2n + 1 merged destinations, up to 4 C(n,2) diagonal classes)
+        // are compacted into one work list, so that all of them go through their chain of dependent
+        // global operations (adjacency, mask, atomic) at the same time, one lane per item
+        if (lane <= ND) sTb[w][lane] = myT;
+        unsigned nitems = 0;
+        {
+            const unsigned bal = __ballot_sync(0xffffffffu, lane <= ND && myT != 0ull);
+            if (lane <= ND && myT) sItem[w][__popc(bal & ((1u << lane) - 1u))] = (uint8_t)lane;
+            nitems = __popc(bal);
+#pragma unroll
+            for (int it = 0; it < (NT - ND + 31) / 32; ++it) {
+                const int t = ND + (int)lane + 32 * it;
+                const bool nz = t < NT && sDiag[w][t - ND] != 0ull;
+                const unsigned bl = __ballot_sync(0xffffffffu, nz);
+                if (nz) sItem[w][nitems + __popc(bl & ((1u << lane) - 1u))] = (uint8_t)(t + 1);   // ND + 1 .. NT: class t
+                nitems += __popc(bl);
             }
         }
-        for (int t = ND + (int)lane; t < NT; t += 32) {
-            const unsigned long long p11 = sDiag[w][t - ND];
-            if (!p11) continue;
-            int j, sj, l2, sl;
-            decode_target<NDIM>(t, j, sj, l2, sl);
-            const int d1 = 2 * j + sj, d2 = 2 * l2 + sl;
-            // diagonal brick: through the adjacency of either face neighbour, else by key
-            uint32_t row = NBR_NONE;
-            const uint32_t r1 = sAdj[w][d1], r2 = sAdj[w][d2];
-            if (r1 != NBR_NONE) row = st.adj[(size_t)r1 * ND + d2];
-            if (row == NBR_NONE && r2 != NBR_NONE) row = st.adj[(size_t)r2 * ND + d1];
-            const uint64_t u1 = 1ull << ((NDIM - 1 - j) * p.bits), u2 = 1ull << ((NDIM - 1 - l2) * p.bits);
-            uint64_t key = sj ? bk + u1 : bk - u1;
-            key = sl ? key + u2 : key - u2;
-            if (GROW) {
-                account(key, grow_apply(p, st, ds, NB0, slots, ND, row, key, p11));
-            } else {
-                if (row == NBR_NONE) row = ht_find(st.table, slots, key);
-                if (row != NBR_NONE) {
-                    const unsigned long long x = p11 & st.mask[row];
-                    if (x) atomicOr((unsigned long long*)&st.keep[row], x);
+        __syncwarp();
+        for (unsigned it = lane; it < nitems; it += 32) {
+            const int code = sItem[w][it];
+            uint32_t row;
+            uint64_t key = bk;
+            unsigned long long bits;
+            if (code <= ND) {                        // own brick or face neighbour code
+                bits = sTb[w][code];
+                row = code == OWN ? b : sAdj[w][code];
+                if (code != OWN) {
+                    const uint64_t u1 = 1ull << ((NDIM - 1 - (code >> 1)) * p.bits);
+                    key = (code & 1) ? bk + u1 : bk - u1;
                 }
+            } else {                                 // diagonal brick of edge class t = code - 1
+                const int t = code - 1;
+                bits = sDiag[w][t - ND];
+                int j, sj, l2, sl;
+                decode_target<NDIM>(t, j, sj, l2, sl);
+                const int d1 = 2 * j + sj, d2 = 2 * l2 + sl;
+                // through the adjacency of either face neighbour, else by key
+                row = NBR_NONE;
+                const uint32_t r1 = sAdj[w][d1], r2 = sAdj[w][d2];
+                if (r1 != NBR_NONE) row = st.adj[(size_t)r1 * ND + d2];
+                if (row == NBR_NONE && r2 != NBR_NONE) row = st.adj[(size_t)r2 * ND + d1];
+                const uint64_t u1 = 1ull << ((NDIM - 1 - j) * p.bits), u2 = 1ull << ((NDIM - 1 - l2) * p.bits);
+                key = sj ? bk + u1 : bk - u1;
+                key = sl ? key + u2 : key - u2;
+                if (!GROW && row == NBR_NONE) row = ht_find(st.table, slots, key);
+            }
+            if (GROW) {
+                account(key, grow_apply(p, st, ds, NB0, slots, ND, row, key, bits));
+            } else if (row != NBR_NONE) {
+                const unsigned long long x = bits & st.mask[row];
+                if (x) atomicOr((unsigned long long*)&st.keep[row], x);
             }
         }
         __syncwarp();
