@@ -349,27 +349,36 @@ def test_paper_lorenz63_scenario_soft_sanity():
 
 
 def test_compare_metrics_and_temporal_convergence():
-    """f1: BC (Eq. 9) and the 1-norm E between two GPU runs on the same grid, checked
-    against the metrics oracle applied to the exported states; and the paper's temporal-convergence
-    protocol: E against a reference run with a very small epsilon decreases with epsilon."""
+    """f1: BC (Eq. 9) and the 1-norm E between two GPU runs on the same grid against
+    the metrics oracle applied to the ORACLE's states of the same two runs; and the paper's
+    temporal-convergence protocol: E against a reference run with a very small
+    epsilon decreases with epsilon."""
     from oracle import metrics_oracle as M
     cfg = W.config0()
 
-    def run(cfl):
+    def run_gpu(cfl):
         g = G(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfl, max_cells=1 << 18)
         g.init_gaussian(cfg["mean"], cfg["cov"])
         g.run(0.05, prune_every=1)
         assert g.time() == 0.05
         return g
 
-    ref = run(0.02)
-    rk, rp = ref.export()
+    def run_oracle(cfl):
+        o = Oracle(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfl)
+        o.init_gaussian(cfg["mean"], cfg["cov"])
+        while o.time() < 0.05:
+            o.step(0.05 - o.time()); o.prune()
+        return o.export()
+
+    ref = run_gpu(0.02)
+    ork, orp = run_oracle(0.02)
     errs = []
     for eps in (1.0, 0.5, 0.2):
-        g = run(eps)
+        g = run_gpu(eps)
         bc, l1 = g.compare(ref)
-        obc, ol1 = M.bc_and_l1(*g.export(), rk, rp)
-        assert bc == pytest.approx(obc, rel=1e-12) and l1 == pytest.approx(ol1, rel=1e-10, abs=1e-13)
+        obc, ol1 = M.bc_and_l1(*run_oracle(eps), ork, orp)
+        # the states agree to 1e-8 (north_star), so the metrics do
+        assert bc == pytest.approx(obc, abs=1e-8) and l1 == pytest.approx(ol1, abs=1e-8)
         bc2, l12 = ref.compare(g)                                   # symmetric
         assert bc2 == pytest.approx(bc, rel=1e-12) and l12 == pytest.approx(l1, rel=1e-10, abs=1e-13)
         assert 0.9 < bc <= 1.0 + 1e-4
@@ -377,7 +386,7 @@ def test_compare_metrics_and_temporal_convergence():
     assert errs[0] > errs[1] > errs[2] > 0.0
     # a run against itself: E = 0; BC = sum of the positive masses = 1 + |negative mass| (A5: negatives are kept)
     bc, l1 = ref.compare(ref)
-    assert l1 == 0.0 and bc == pytest.approx(rp[rp > 0].sum(), rel=1e-12) and abs(bc - 1.0) < 1e-4
+    assert l1 == 0.0 and bc == pytest.approx(orp[orp > 0].sum(), abs=1e-8) and abs(bc - 1.0) < 1e-4
     print("temporal convergence, E(eps = 1, 0.5, 0.2) vs eps = 0.02:", errs)
 
 
@@ -392,12 +401,13 @@ def test_marginals_of_the_6d_pdf():
     g = G(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfg["cfl"], max_cells=cfg["max_cells"])
     g.init_gaussian(cfg["mean"], cfg["cov"])
     g.run(1e300, max_steps=6, prune_every=5)
-    keys, p = g.export()
+    o, _ = oracle_run(cfg, steps=6)
+    keys, p = o.export()                               # the oracle's state: the expected marginals come from it
     for dims in ([0, 1, 2], [3, 4, 5], [4], [5, 0], [0, 1, 2, 3, 4, 5]):
         mk, mp = g.marginal(dims)
         ok, op = MO.marginal(keys, p, dims)
         assert np.array_equal(mk, ok), dims
-        assert np.max(np.abs(mp - op)) <= 1e-12 * op.max()
+        assert np.max(np.abs(mp - op)) <= 1e-10 * op.max()
         assert mp.sum() == pytest.approx(1.0, abs=1e-12)
     # buffer contract: count only, too small a buffer
     d = (C.c_int * 3)(0, 1, 2)
