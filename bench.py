@@ -187,6 +187,12 @@ def run_cfg4(args):
             p_ins, t_ins = timed(lambda: ht.insert(kt, idx))
             p_hit, t_hit = timed(lambda: ht.lookup(kt, idx))
             p_nb, t_nb = timed(lambda: ht.lookup(q, qo))
+            coop = {}
+            for wdt in (4, 32):
+                pc, tc = timed(lambda: ht.lookup_coop(q, qo, wdt))
+                ph, th = timed(lambda: ht.lookup_coop(kt, idx, wdt))
+                coop[f"w{wdt}"] = {"neighbours_Mops": q.numel() / tc / 1e6, "hit_Mops": K / th / 1e6,
+                                   "probes_equal_scalar": bool(pc == p_nb and ph == p_hit)}
             kept, t_cmp = timed(lambda: ht.compact(kt, dele))
             ht.close()
             rows.append({"keys": K, "alpha": alpha,
@@ -194,6 +200,7 @@ def run_cfg4(args):
                          "lookup_hit": {"probes_per_op": p_hit / K, "Mops": K / t_hit / 1e6, "GBps": K * (8 + 16 * p_hit / K + 4) / t_hit / 1e9},
                          "lookup_neighbours": {"probes_per_op": p_nb / q.numel(), "Mops": q.numel() / t_nb / 1e6,
                                                "GBps": q.numel() * (8 + 16 * p_nb / q.numel() + 4) / t_nb / 1e9},
+                         "cooperative_probing": coop,
                          "delete30_compact_rebuild": {"survivors": kept, "Mkeys_per_s": K / t_cmp / 1e6}})
     print(json.dumps({"metric": "hashtable / compaction microbench (BASELINE config 4)", "unit": "probes/op, M ops/s, GB/s",
                       "n_gpus": 1, "data": "synthetic", "config": {"workload": "cfg4_hashtable", "keys": args.cfg4_keys},

@@ -173,6 +173,10 @@ int gbees_ht_destroy(gbees_ht* ht);
 int gbees_ht_insert(gbees_ht* ht, const uint64_t* keys, int64_t k, uint32_t* idx_out, uint64_t* probes /*host*/);
 /* out[i] = pool index of query[i] or 0xFFFFFFFF */
 int gbees_ht_lookup(gbees_ht* ht, const uint64_t* query, int64_t k, uint32_t* out, uint64_t* probes /*host*/);
+/* the same lookup with cooperative probing (north_star: "warp-cooperative probing"): a tile of `width`
+ * lanes (4, 8 or 32) inspects `width` consecutive slots per round for one query. Same answers and the
+ * same probe count as gbees_ht_lookup. */
+int gbees_ht_lookup_coop(gbees_ht* ht, const uint64_t* query, int64_t k, uint32_t* out, uint64_t* probes /*host*/, int width);
 /* delete keys[i] where del[i] != 0: decoupled-lookback scan + stable compaction of keys (in place)
  * + table rebuild. *k_out = survivors. */
 int gbees_ht_compact(gbees_ht* ht, uint64_t* keys, const uint8_t* del, int64_t k, int64_t* k_out /*host*/);

@@ -233,6 +233,7 @@ class HashTable:
         L.gbees_ht_insert.argtypes = [vp, vp, C.c_int64, vp, C.POINTER(C.c_uint64)]
         L.gbees_ht_lookup.argtypes = [vp, vp, C.c_int64, vp, C.POINTER(C.c_uint64)]
         L.gbees_ht_compact.argtypes = [vp, vp, vp, C.c_int64, C.POINTER(C.c_int64)]
+        L.gbees_ht_lookup_coop.argtypes = [vp, vp, C.c_int64, vp, C.POINTER(C.c_uint64), C.c_int]
         self._h = vp()
         rc = L.gbees_ht_create(C.byref(self._h), int(slots), int(device))
         if rc:
@@ -260,6 +261,14 @@ class HashTable:
                                    out_t.data_ptr() if out_t is not None else None, C.byref(pr))
         if rc:
             raise GbeesError(rc, "gbees_ht_lookup failed")
+        return pr.value
+
+    def lookup_coop(self, query_t, out_t=None, width=4):
+        pr = C.c_uint64()
+        rc = lib().gbees_ht_lookup_coop(self._h, query_t.data_ptr(), int(query_t.numel()),
+                                        out_t.data_ptr() if out_t is not None else None, C.byref(pr), int(width))
+        if rc:
+            raise GbeesError(rc, "gbees_ht_lookup_coop failed")
         return pr.value
 
     def compact(self, keys_t, del_t):

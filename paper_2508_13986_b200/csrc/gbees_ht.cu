@@ -56,6 +56,53 @@ __global__ void __launch_bounds__(TPB) k_ht_lookup(const ulonglong2* table, uint
     add_probes(probes, np);
 }
 
+// Cooperative probing (north_star: "warp-cooperative probing"): a tile of W lanes serves one query and
+// inspects W consecutive 16-byte slots per round (W = 4: 64 bytes = two sectors; W = 32: 512 bytes),
+// so a long probe chain costs ceil(len / W) dependent memory rounds instead of len. The lanes of a
+// tile take the tile's queries in turn (lane t of the tile owns query t). probes = slots up to and
+// including the one that ended the search, as in the scalar kernel.
+template <int W>
+__global__ void __launch_bounds__(TPB) k_ht_lookup_coop(const ulonglong2* __restrict__ table, uint64_t slots, const uint64_t* q,
+                                                        int64_t k, uint32_t* out, unsigned long long* probes) {
+    const unsigned lane = threadIdx.x & 31, tl = lane % W, tbase = lane - tl;
+    const unsigned tmask = (W == 32 ? 0xffffffffu : ((1u << W) - 1u) << tbase);
+    unsigned np = 0;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    const int64_t kk = (k + stride - 1) / stride * stride;      // all lanes of a tile iterate together
+    for (int64_t i = gtid(); i < kk; i += stride) {
+        const bool have = i < k;
+        const uint64_t myq = have ? q[i] : 0ull;
+        uint32_t myres = NBR_NONE;
+        for (int t = 0; t < W; ++t) {
+            const uint64_t key = __shfl_sync(tmask, myq, tbase + t);
+            const bool valid = __shfl_sync(tmask, (int)have, tbase + t) != 0;
+            if (!valid) continue;                                 // uniform within the tile
+            uint64_t s = home_slot(key, slots);
+            uint32_t res = NBR_NONE;
+            for (;;) {
+                uint64_t ss = s + tl;
+                if (ss >= slots) ss -= slots;
+                const ulonglong2 e = table[ss];
+                const unsigned hit = __ballot_sync(tmask, e.x == key) >> tbase;
+                const unsigned emp = __ballot_sync(tmask, e.x == KEY_EMPTY) >> tbase;
+                const unsigned ev = (hit | emp) & (W == 32 ? 0xffffffffu : (1u << W) - 1u);
+                if (ev) {
+                    const int first = __ffs((int)ev) - 1;
+                    if ((hit >> first) & 1u) res = (uint32_t)__shfl_sync(tmask, (unsigned)e.y, tbase + first);
+                    if ((int)tl == t) np += (unsigned)first + 1u;
+                    break;
+                }
+                if ((int)tl == t) np += W;
+                s += W;
+                if (s >= slots) s -= slots;
+            }
+            if ((int)tl == t) myres = res;
+        }
+        if (have && out) out[i] = myres;
+    }
+    add_probes(probes, np);
+}
+
 __global__ void __launch_bounds__(TPB) k_ht_compact(const uint64_t* keys, const uint8_t* del, uint32_t k, uint64_t* keys2,
                                                     unsigned long long* tile_state, unsigned int* tile_counter,
                                                     uint32_t* total) {
@@ -122,6 +169,20 @@ int gbees_ht_lookup(gbees_ht* h, const uint64_t* q, int64_t k, uint32_t* out, ui
     HT_CU(cudaSetDevice(h->device));
     HT_CU(cudaMemset(h->probes, 0, 8));
     k_ht_lookup<<<h->grid, TPB>>>(h->table, h->slots, q, k, out, h->probes);
+    HT_CU(cudaGetLastError());
+    unsigned long long pr = 0;
+    HT_CU(cudaMemcpy(&pr, h->probes, 8, cudaMemcpyDeviceToHost));
+    if (probes) *probes = pr;
+    return GBEES_OK;
+}
+
+int gbees_ht_lookup_coop(gbees_ht* h, const uint64_t* q, int64_t k, uint32_t* out, uint64_t* probes, int width) {
+    if (!h || !q || k < 0 || (width != 4 && width != 8 && width != 32)) return GBEES_ERR_ARG;
+    HT_CU(cudaSetDevice(h->device));
+    HT_CU(cudaMemset(h->probes, 0, 8));
+    if (width == 4) k_ht_lookup_coop<4><<<h->grid, TPB>>>(h->table, h->slots, q, k, out, h->probes);
+    else if (width == 8) k_ht_lookup_coop<8><<<h->grid, TPB>>>(h->table, h->slots, q, k, out, h->probes);
+    else k_ht_lookup_coop<32><<<h->grid, TPB>>>(h->table, h->slots, q, k, out, h->probes);
     HT_CU(cudaGetLastError());
     unsigned long long pr = 0;
     HT_CU(cudaMemcpy(&pr, h->probes, 8, cudaMemcpyDeviceToHost));

@@ -76,6 +76,12 @@ def test_gpu_table_insert_lookup_compact(alpha):
     assert np.array_equal(got, found)
     assert found.mean() < 0.01
     assert probes_q / len(q) == pytest.approx(gu, rel=0.05)
+    # cooperative probing (tiles of 4, 8, 32 lanes): same answers, same probe counts
+    for width in (4, 8, 32):
+        qo2 = torch.empty(len(q), dtype=torch.int32, device="cuda")
+        assert ht.lookup_coop(qt, qo2, width) == probes_q and torch.equal(qo2, qo)
+        out3 = torch.empty(K, dtype=torch.int32, device="cuda")
+        assert ht.lookup_coop(kt, out3, width) == probes_hit and torch.equal(out3, idx)
     # delete 30 %, compact (stable), rebuild
     dele = (rng.random(K) < 0.3).astype(np.uint8)
     dt_ = torch.from_numpy(dele).cuda()
