@@ -1,5 +1,5 @@
 // Host side of the C ABI in include/gbees.h: context, launches, error handling.
-// All arithmetic of the method runs in the kernels of gbees_kernels.cuh; the host only computes
+// All arithmetic of the method runs in the kernels of gbees_brick.cuh; the host only computes
 // the launch-invariant inputs of init_gaussian / correct (an n x n Cholesky inverse, n <= 6).
 #include <cmath>
 #include <cstdio>

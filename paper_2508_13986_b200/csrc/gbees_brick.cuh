@@ -1,7 +1,7 @@
 // Kernels of the GBEES prediction step on the dense-brick store.
-// Every phase is a grid-stride __device__ function, so the same code runs as a stream of small
-// launches (gbees_step / gbees_prune) or inside the persistent cooperative loop (gbees_run,
-// PAPER.md:170-172). Semantics: DESIGN.md D1-D5 (= SURVEY.md 8(c)).
+// Every phase is a grid-stride __device__ function, so the same code runs as a stream of launches
+// (gbees_step / gbees_prune / gbees_run) or inside the persistent single-cluster loop for small
+// grids (k_run_small). Semantics: DESIGN.md D1-D5 (= SURVEY.md 8(c)).
 //
 // Brick geometry: 64 cell slots per brick, 2^K_j cells along dimension j (sum K_j = 6; n = 6: a
 // 2x2x2x2x2x2 box). Local index l = concatenation of the low K_j bits of every coordinate, dim 0
@@ -86,8 +86,8 @@ __device__ __forceinline__ void decode_target(int t, int& j, int& sj, int& l, in
 // Bit-parallel per brick: one warp turns the sources' outflow flags into 2n slot masks O_d, then
 // every lane takes target classes t (a face step or a pair of steps), ANDs the masks of the steps
 // involved, shifts the result to the target slots and splits it by destination brick (own, face
-// neighbour, diagonal). Masks bound for the own brick and the 2n face neighbours are merged in
-// shared memory, so a brick costs O(2n + diagonals) global atomics instead of O(cells x targets).
+// neighbour, diagonal). Masks bound for the own brick and the 2n face neighbours are merged with
+// warp OR-reductions, so a brick costs O(2n + diagonals) global atomics instead of O(cells x targets).
 template <int NDIM>
 __device__ __forceinline__ unsigned long long edge_mask(int j, int side) {   // slots whose step (j, side) leaves the brick
     unsigned long long e = 0ull;
