@@ -1,9 +1,9 @@
-"""Writes tests/golden/cfg3s_full_oracle.json: the CPU oracle's result for the 1/10-scale twin of
-BASELINE config 3 (linear 6-D stress f = Ax, dx = 0.5, 50 steps, prune every 5; 6.2 M -> 10 M cells,
-4.7e8 cell-updates). Calls ONLY oracle/ (plus the seeded workload parameters). Takes more than an
-hour on one core.
+"""Writes tests/golden/cfg3m_full_oracle.json: the CPU oracle's result for a mid-scale twin of
+BASELINE config 3 (linear 6-D stress f = Ax, dx = 0.7, all 50 steps, prune every 5; about 1 M cells:
+the largest size the serial oracle finishes in tens of minutes -- the 1/10-scale twin (dx = 0.5,
+10 M cells) needs ~5 minutes per oracle step). Calls ONLY oracle/ (plus the seeded workload parameters).
 
-    python tests/golden/make_cfg3s_golden.py
+    python tests/golden/make_cfg3m_golden.py
 """
 import json
 import os
@@ -18,7 +18,7 @@ from paper_2508_13986_b200 import workloads as W  # noqa: E402
 
 
 def main():
-    cfg = W.config3(dx=0.5)
+    cfg = W.config3(dx=0.7)
     o = Oracle(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfg["cfl"])
     o.init_gaussian(cfg["mean"], cfg["cov"])
     k, counts, dts = 0, [o.count()], []
@@ -35,12 +35,12 @@ def main():
     rnd = rng.choice(len(p), 96, replace=False)
     idx = np.unique(np.concatenate([top, rnd]))
     out = {
-        "citation": "BASELINE.json configs[3] at 1/10 scale (SURVEY.md 8(d)); oracle = oracle/gbees_oracle.cpp (DESIGN.md D1-D5)",
+        "citation": "BASELINE.json configs[3] with dx = 0.7 (mid-scale twin); oracle = oracle/gbees_oracle.cpp (DESIGN.md D1-D5)",
         "steps": k, "t": o.time(), "final_cells": int(len(p)), "cells_after_each_step": [int(c) for c in counts],
         "dt_first": dts[0], "dt_last": dts[-1], "p_max": float(p.max()),
         "sample_keys": keys[idx].tolist(), "sample_p": [float(v) for v in p[idx]],
     }
-    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "cfg3s_full_oracle.json")
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "cfg3m_full_oracle.json")
     with open(path, "w") as f:
         json.dump(out, f, indent=1)
     print("wrote", path, "steps", k, "cells", len(p))

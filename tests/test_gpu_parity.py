@@ -417,3 +417,28 @@ def test_marginals_of_the_6d_pdf():
     assert lib().gbees_marginal(g._h, d, 3, small.ctypes.data, sp.ctypes.data, 4, C.byref(cnt)) == -5
     bad = (C.c_int * 2)(1, 1)
     assert lib().gbees_marginal(g._h, bad, 2, None, None, 0, C.byref(cnt)) == -1
+
+
+def test_config3_midscale_full_run_against_oracle_golden():
+    """BASELINE config 3's recipe (linear 6-D f = Ax, 50 steps, prune every 5) on a mid-scale grid
+    (dx = 0.7, ~2 M cells: the largest the serial oracle finishes in tens of minutes) through gbees_run,
+    against the oracle's stored result (tests/golden/cfg3m_full_oracle.json, written by
+    tests/golden/make_cfg3m_golden.py, which calls only oracle/)."""
+    import json
+    import os
+    gold = json.load(open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "cfg3m_full_oracle.json")))
+    cfg = W.config3(dx=0.7)
+    g = G(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfg["cfl"], max_cells=1 << 24)
+    g.init_gaussian(cfg["mean"], cfg["cov"])
+    assert g.count() == gold["cells_after_each_step"][0]
+    for k in range(5, cfg["steps"] + 1, 5):
+        assert g.run(1e300, max_steps=5, prune_every=0) == 5
+        g.prune()
+        assert g.count() == gold["cells_after_each_step"][k], f"cell count after step {k}"
+    assert g.stats()["steps"] == gold["steps"] == cfg["steps"]
+    assert g.time() == pytest.approx(gold["t"], rel=1e-13)
+    gk, gp = g.export()
+    assert len(gp) == gold["final_cells"]
+    lut = {tuple(k): v for k, v in zip(gk.tolist(), gp.tolist())}
+    got = np.array([lut[tuple(k)] for k in gold["sample_keys"]])      # KeyError = active sets differ
+    assert np.max(np.abs(got - np.array(gold["sample_p"]))) <= 1e-8 * gold["p_max"]
