@@ -442,3 +442,47 @@ def test_config3_midscale_full_run_against_oracle_golden():
     lut = {tuple(k): v for k, v in zip(gk.tolist(), gp.tolist())}
     got = np.array([lut[tuple(k)] for k in gold["sample_keys"]])      # KeyError = active sets differ
     assert np.max(np.abs(got - np.array(gold["sample_p"]))) <= 1e-8 * gold["p_max"]
+
+
+def test_config3_tenth_scale_properties_at_full_size():
+    """BASELINE config 3 at 1/10 scale (6-10 M cells; the oracle needs ~5 min per step there, so no
+    element-wise oracle comparison): properties that hold at any size. (1) through gbees_run, the launch
+    configuration bench.py times: masses sum to 1, no key twice, count == stats. (2) P13 reflection
+    symmetry at scale: the problem mirrored in axis 0 (A -> D A D, D = diag(-1, 1, ..., 1); N(0, I) is
+    symmetric) gives the mirrored key set and the same masses. Eq. (8) as printed looks at LOWER faces
+    only, so the CFL step itself is not mirror-symmetric: both runs take the same capped dt."""
+    cfg = W.config3(dx=0.5)
+    A = np.array(cfg["params"]).reshape(6, 6)
+    D = np.diag([-1.0, 1, 1, 1, 1, 1])
+
+    def make(params):
+        g = G(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], params, cfl=cfg["cfl"], max_cells=1 << 25)
+        g.init_gaussian(cfg["mean"], cfg["cov"])
+        return g
+
+    g = make(A.ravel())
+    assert g.run(1e300, max_steps=10, prune_every=5) == 10
+    k0, p0 = g.export()
+    st = g.stats()
+    assert st["n_cells"] == len(p0) > 6_000_000 and st["prunes"] == 2
+    assert p0.sum() == pytest.approx(1.0, abs=1e-11)
+    assert not np.any(np.all(k0[1:] == k0[:-1], axis=1))            # sorted export: equal neighbours = duplicate key
+    cap = 0.7 * st["dt"]
+    g.close()
+
+    def capped(params):
+        g = make(params)
+        for k in range(1, 7):
+            assert g.step(cap) == cap
+            if k % 3 == 0:
+                g.prune()
+        out = g.export()
+        g.close()
+        return out
+
+    k1, p1 = capped(A.ravel())
+    k2, p2 = capped((D @ A @ D).ravel())
+    k2m = k2.copy(); k2m[:, 0] = -k2m[:, 0]
+    order = np.lexsort(k2m.T[::-1])
+    assert np.array_equal(k2m[order], k1)
+    assert np.max(np.abs(p2[order] - p1)) <= 1e-10 * p1.max()
