@@ -486,3 +486,22 @@ def test_config3_tenth_scale_properties_at_full_size():
     order = np.lexsort(k2m.T[::-1])
     assert np.array_equal(k2m[order], k1)
     assert np.max(np.abs(p2[order] - p1)) <= 1e-10 * p1.max()
+
+
+@pytest.mark.parametrize("prune_every,max_steps", [(3, 17), (0, 9)])
+def test_small_grid_persistent_loop_prune_cadence(prune_every, max_steps):
+    """a9 on a small grid (single-cluster persistent loop): prune cadences other than 1 and a step limit
+    that is not a multiple of the cadence, against the oracle's step / prune sequence; then the context
+    keeps working call by call."""
+    cfg = W.config0()
+    cfg.update(prune_every=prune_every)
+    g = G(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfg["cfl"], max_cells=cfg["max_cells"])
+    g.init_gaussian(cfg["mean"], cfg["cov"])
+    assert g.run(1e300, max_steps=max_steps, prune_every=prune_every) == max_steps
+    o, _ = oracle_run(cfg, steps=max_steps)
+    assert g.time() == pytest.approx(o.time(), rel=1e-14)
+    compare_states(*g.export(), *o.export(), cfg["thresh"], 1e-9, what="small-grid run")
+    assert g.stats()["launches"] < 40                                  # one launch for the loop, not 4 per step
+    assert abs(g.step() - o.step()) <= 1e-14
+    g.prune(); o.prune()
+    compare_states(*g.export(), *o.export(), cfg["thresh"], 1e-9, what="small-grid run + step + prune")
