@@ -23,6 +23,7 @@ def lib():
         L.gbeeso_prune.argtypes = [vp]
         L.gbeeso_correct.argtypes = [vp, dp, dp]
         L.gbeeso_correct_linear.argtypes = [vp, dp, C.c_int, dp, dp]
+        L.gbeeso_correct_range.argtypes = [vp, dp, C.c_double, C.c_double]
         L.gbeeso_export.argtypes = [vp, ip, dp, C.c_int64, C.POINTER(C.c_int64)]
         L.gbeeso_count.argtypes = [vp]
         L.gbeeso_count.restype = C.c_int64
@@ -107,6 +108,11 @@ class Oracle:
         ya, yp = _d(y)
         _, rp = _d(R)
         _chk(lib().gbeeso_correct_linear(self._h, hp, int(ya.size), yp, rp), "correct_linear")
+
+    def correct_range(self, s, y, sigma):
+        """Eq. (4) with the non-linear range measurement y = ||x - s|| + v, v ~ N(0, sigma^2)."""
+        _, sp = _d(s)
+        _chk(lib().gbeeso_correct_range(self._h, sp, float(y), float(sigma)), "correct_range")
 
     def count(self):
         return int(lib().gbeeso_count(self._h))

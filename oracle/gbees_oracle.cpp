@@ -516,6 +516,22 @@ int correct_linear(Oracle& o, const double* H, int m, const double* y, const dou
     return normalise(o);
 }
 
+// ---- f2, a NON-linear measurement: the range to a point s, y = ||x - s||_2 + v, v ~ N(0, sigma^2).
+// Eq. (4): P_c <- P_c * exp(-1/2 ((y - ||x_c - s||) / sigma)^2), then normalise.
+int correct_range(Oracle& o, const double* s, double y, double sigma) {
+    if (!(sigma > 0.0)) return -3;
+    for (size_t i = 0; i < o.key.size(); ++i) {
+        double r2 = 0.0;
+        for (int j = 0; j < o.n; ++j) {
+            const double d = (o.mu[j] + (double)o.key[i][j] * o.h[j]) - s[j];
+            r2 += d * d;
+        }
+        const double e = (y - std::sqrt(r2)) / sigma;
+        o.P[i] *= std::exp(-0.5 * e * e);
+    }
+    return normalise(o);
+}
+
 }  // namespace
 
 // ================================ C ABI (host pointers only) ====================================
@@ -577,6 +593,7 @@ int gbeeso_import(void* h, const double* origin, const int32_t* keys, const doub
 int gbeeso_step(void* h, double* dt) { return step(*(Oracle*)h, dt); }
 int gbeeso_prune(void* h) { return prune(*(Oracle*)h); }
 int gbeeso_correct(void* h, const double* z, const double* R) { return correct(*(Oracle*)h, z, R); }
+int gbeeso_correct_range(void* h, const double* s, double y, double sigma) { return correct_range(*(Oracle*)h, s, y, sigma); }
 int gbeeso_correct_linear(void* h, const double* H, int m, const double* y, const double* R) {
     return correct_linear(*(Oracle*)h, H, m, y, R);
 }

@@ -346,6 +346,30 @@ def test_P10b_partial_state_correction_direct_and_kalman():
     assert np.array_equal(a.export()[1], b.export()[1])
 
 
+def test_P10c_range_measurement_direct_and_1d_reduction():
+    """f2, non-linear h(x) = ||x - s||: direct definition of Eq. (4); in 1-D with s far to the left the range
+    is x - s, so the update equals the linear one with H = (1), y' = y + s; the posterior concentrates on
+    the sphere of radius y (mean range -> y as sigma -> 0)."""
+    n, dx = 3, 0.25
+    mu0, cov0 = np.array([1.0, -2.0, 0.5]), np.diag([1.0, 0.6, 0.8])
+    s0, y, sig = np.array([-1.0, 0.5, 0.0]), 3.2, 0.4
+    o = Oracle(n, [dx] * n, 1e-9, 4, [0.0] * n)
+    o.init_gaussian(mu0, cov0)
+    keys, p0 = o.export()
+    o.correct_range(s0, y, sig)
+    k1, p1 = o.export()
+    r = np.linalg.norm(mu0 + keys * dx - s0, axis=1)
+    L = np.exp(-0.5 * ((y - r) / sig) ** 2)
+    want = p0 * L / (p0 * L).sum()
+    assert np.array_equal(keys, k1) and np.max(np.abs(p1 - want)) <= 1e-13 * want.max()
+    o2 = Oracle(n, [dx] * n, 1e-9, 4, [0.0] * n); o2.init_gaussian(mu0, cov0); o2.correct_range(s0, y, 0.05)
+    k2, p2 = o2.export()
+    assert abs((p2 * np.linalg.norm(mu0 + k2 * dx - s0, axis=1)).sum() - y) < 0.02
+    a = Oracle(1, [0.1], 1e-9, 4, [0.0]); a.init_gaussian([0.3], [[0.5]]); a.correct_range([-50.0], 50.9, 0.3)
+    b = Oracle(1, [0.1], 1e-9, 4, [0.0]); b.init_gaussian([0.3], [[0.5]]); b.correct_linear([[1.0]], [0.9], [[0.09]])
+    assert np.max(np.abs(a.export()[1] - b.export()[1])) <= 1e-12
+
+
 def test_A8_init_gaussian_set_and_values():
     n, dx, thr = 3, 0.5, 2e-5
     cov = np.array([[1.0, 0.3, 0.0], [0.3, 0.8, -0.2], [0.0, -0.2, 1.1]])
