@@ -125,6 +125,11 @@ int gbees_correct(gbees_ctx* ctx, const double* z, const double* R);
  * renormalise. H [m*n row-major], y [m], R [m*m row-major SPD]: host; 1 <= m <= 6. Does not prune. */
 int gbees_correct_linear(gbees_ctx* ctx, const double* H, int m, const double* y, const double* R);
 
+/* Eq. (4) with a NON-linear measurement, the range to the point s: y = ||x - s||_2 + v, v ~ N(0, sigma^2):
+ * P_c <- P_c * exp(-1/2 ((y - ||x_c - s||) / sigma)^2), renormalise. s [n]: host; sigma > 0 (else
+ * GBEES_ERR_NOT_SPD). Does not prune. */
+int gbees_correct_range(gbees_ctx* ctx, const double* s, double y, double sigma);
+
 /* Distribution metrics between two contexts on the SAME grid (same n, dx, origin, device; else
  * GBEES_ERR_ARG): *bc = sum_c sqrt(Pa_c Pb_c) (Bhattacharyya coefficient, Eq. 9) and
  * *l1 = sum_c |Pa_c - Pb_c| (the paper's 1-norm E of PAPER.md:362-366 in cell masses), over the union

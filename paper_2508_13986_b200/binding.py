@@ -59,6 +59,7 @@ def lib():
         L.gbees_time.argtypes = [vp, dp]
         L.gbees_correct_linear.argtypes = [vp, dp, C.c_int, dp, dp]
         L.gbees_compare.argtypes = [vp, vp, dp, dp]
+        L.gbees_correct_range.argtypes = [vp, dp, C.c_double, C.c_double]
         L.gbees_marginal.argtypes = [vp, C.POINTER(C.c_int), C.c_int, vp, vp, C.c_int64, C.POINTER(C.c_int64)]
         L.gbees_stats.argtypes = [vp, C.POINTER(Stats)]
         L.gbees_profile.argtypes = [vp, C.c_int, dp, C.POINTER(C.c_int64)]
@@ -145,6 +146,10 @@ class Gbees:
         ya, yp = _d(y)
         _, rp = _d(R)
         self._chk(lib().gbees_correct_linear(self._h, hp, int(ya.size), yp, rp))
+
+    def correct_range(self, s, y, sigma):
+        _, sp = _d(s)
+        self._chk(lib().gbees_correct_range(self._h, sp, float(y), float(sigma)))
 
     def compare(self, other):
         """(BC, E) between this context and another one on the same grid (Eq. 9 and the 1-norm of PAPER.md:362-366)."""

@@ -193,6 +193,8 @@ __global__ void __launch_bounds__(TPB) k_init_gaussian(GP, const __grid_constant
 template <int NDIM>
 __global__ void __launch_bounds__(TPB) k_correct(GP, const __grid_constant__ GaussArgs g) { ST; phase_correct<NDIM>(p, st, ds, g); }
 template <int NDIM>
+__global__ void __launch_bounds__(TPB) k_correct_range(GP, const __grid_constant__ GaussArgs g) { ST; phase_correct_range<NDIM>(p, st, ds, g); }
+template <int NDIM>
 __global__ void __launch_bounds__(TPB) k_correct_linear(GP, const __grid_constant__ GaussArgs g) { ST; phase_correct_linear<NDIM>(p, st, ds, g); }
 template <int NDIM>
 __global__ void __launch_bounds__(TPB) k_compare(const __grid_constant__ Params p, const __grid_constant__ Store a_in, const DevState* da,
@@ -717,6 +719,28 @@ int gbees_correct(gbees_ctx* c, const double* z, const double* R) {
     phase(c, GBEES_PH_CORRECT, 3, [&] {
         dispatch_n(c, [&](auto N_) {
             k_correct<decltype(N_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, g);
+            return GBEES_OK;
+        });
+        k_sum<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 0, 0);
+        k_finish<<<1, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, c->grid, 1, 0);
+    });
+    CU(cudaGetLastError());
+    return sync_state(c);
+}
+
+int gbees_correct_range(gbees_ctx* c, const double* s, double y, double sigma) {
+    if (!c || !s) return GBEES_ERR_ARG;
+    if (!(sigma > 0.0)) return GBEES_ERR_NOT_SPD;
+    if (c->sticky) return c->sticky;
+    CU(cudaSetDevice(c->device));
+    GaussArgs g;
+    std::memset(&g, 0, sizeof(g));
+    for (int j = 0; j < c->p.n; ++j) g.v[j] = s[j];
+    g.norm = y;
+    g.inv[0] = 1.0 / sigma;
+    phase(c, GBEES_PH_CORRECT, 3, [&] {
+        dispatch_n(c, [&](auto N_) {
+            k_correct_range<decltype(N_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, g);
             return GBEES_OK;
         });
         k_sum<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 0, 0);

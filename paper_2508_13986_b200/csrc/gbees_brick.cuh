@@ -899,6 +899,30 @@ __device__ void phase_correct_linear(const Params& p, const Store& st, DevState*
     }
 }
 
+// f2, a non-linear measurement: the range to a point s (g.v), y = ||x - s|| + v, v ~ N(0, sigma^2):
+// Q_c *= exp(-1/2 ((y - ||x_c - s||) / sigma)^2)            (Eq. 4; g.norm = y, g.inv[0] = 1 / sigma)
+template <int NDIM>
+__device__ void phase_correct_range(const Params& p, const Store& st, DevState* ds, const GaussArgs& g) {
+    const uint32_t NB = min(ds->NB, p.capB);
+    const uint64_t items = (uint64_t)NB * 64;
+    for (uint64_t i = gtid(); i < items; i += gthreads()) {
+        const uint32_t b = (uint32_t)(i >> 6);
+        const int l = (int)(i & 63);
+        if (!((st.mask[b] >> l) & 1ull)) continue;
+        int32_t B[NDIM], c[NDIM];
+        unpack<NDIM>(p, st.bkey[b], B);
+        cell_coords<NDIM>(B, l, c);
+        double r2 = 0.0;
+#pragma unroll
+        for (int j = 0; j < NDIM; ++j) {
+            const double d = (p.mu[j] + (double)c[j] * p.h[j]) - g.v[j];
+            r2 += d * d;
+        }
+        const double e = (g.norm - sqrt(r2)) * g.inv[0];
+        st.Q[i] *= exp(-0.5 * e * e);
+    }
+}
+
 // f1, distribution metrics between two contexts on the same grid (same n, dx, origin):
 //   BC = sum_c sqrt(Pa_c Pb_c)  (Eq. 9),  E = sum_c |Pa_c - Pb_c|  (masses).
 // One warp per brick of A looks the brick up in B's table (hash join over BRICK keys); per-block

@@ -320,6 +320,21 @@ def test_correct_linear_partial_state_parity():
         compare_states(*g.export(), *o.export(), cfg["thresh"], 1e-10, what="correct_linear + prune + step")
 
 
+def test_correct_range_nonlinear_measurement_parity():
+    """f2, non-linear h(x) = ||x - s||: GPU against the oracle, then a prune and a step."""
+    cfg = W.config0()
+    g = G(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfg["cfl"], max_cells=cfg["max_cells"])
+    o = Oracle(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfg["cfl"])
+    g.init_gaussian(cfg["mean"], cfg["cov"]); o.init_gaussian(cfg["mean"], cfg["cov"])
+    for _ in range(2):
+        g.step(); o.step(); g.prune(); o.prune()
+    s0 = np.array([-9.0, -8.5, 12.0])
+    g.correct_range(s0, 3.0, 0.5); o.correct_range(s0, 3.0, 0.5)
+    compare_states(*g.export(), *o.export(), cfg["thresh"], 1e-10, what="after correct_range")
+    g.prune(); o.prune(); g.step(); o.step()
+    compare_states(*g.export(), *o.export(), cfg["thresh"], 1e-10, what="correct_range + prune + step")
+
+
 def test_paper_lorenz63_scenario_soft_sanity():
     """The paper's own Lorenz '63 run: z-shifted form with (sigma, b, r) = (4, 1, 48),
     h = 0.5, dt = 1.0 x CFL, t in [0, 2], one measurement y = x3 = -8 (sigma_y = 1) at t = 1. GPU == oracle
