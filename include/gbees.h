@@ -81,11 +81,11 @@ enum {
     GBEES_PH_PASSB,     /* a5+a6: fetch neighbour-brick fluxes, update, mass sum, dt/t bookkeeping (k_flux2) */
     GBEES_PH_MARK,      /* a7: prune marking */
     GBEES_PH_COMPACT,   /* a7: decoupled-lookback scan over bricks + row compaction */
-    GBEES_PH_REBUILD,   /* a7/a0: hashtable clear + re-insert */
-    GBEES_PH_RELINK,    /* adjacency + CFL maximum for all cells, mass sum, renormalise */
+    GBEES_PH_REBUILD,   /* a7/a0: hashtable clear + re-insert (in a prune: + CFL maximum, mass sum, cell count) */
+    GBEES_PH_RELINK,    /* adjacency for all bricks (in a prune: + renormalise by the last block) */
     GBEES_PH_SUM,       /* a6: mass sum + renormalise outside a step */
     GBEES_PH_CORRECT,   /* a8 */
-    GBEES_PH_RUN,       /* a9: persistent cooperative step loop (whole launch) */
+    GBEES_PH_RUN,       /* a9: persistent single-cluster step loop for small grids (whole launch; not used while profiling) */
     GBEES_PHASES
 };
 
@@ -160,7 +160,8 @@ int gbees_time(gbees_ctx* ctx, double* t /*host*/);
 int gbees_stats(gbees_ctx* ctx, gbees_stats_t* out /*host*/);
 /* Read-and-reset the per-phase accumulators (phase_ms, phase_launches: host [GBEES_PHASES],
  * nullable), then switch CUDA-event timing of every phase on/off. Synchronises the stream.
- * Launch counts are always kept; milliseconds only while profiling is enabled. */
+ * Launch counts are always kept; milliseconds only while profiling is enabled. While profiling is on
+ * gbees_run always uses the per-phase launches (never the single-launch loop for small grids). */
 int gbees_profile(gbees_ctx* ctx, int enable, double* phase_ms, int64_t* phase_launches);
 /* Kept for ABI stability: per-phase device timers of the former persistent kernel. The phases of
  * gbees_run are separate launches now and are timed by gbees_profile; this call returns zeros.
