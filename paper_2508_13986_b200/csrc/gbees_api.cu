@@ -152,15 +152,23 @@ __global__ void __launch_bounds__(TPB) k_run_small(GP, int prune_every, int no_g
         cl.sync();
         phase_prune_scan(p, st, ds);
         cl.sync();
+        // (the counts are final after the scan: snapshot them before the barrier that ends the move)
+        const uint32_t nb_old = min(ds->NB, p.capB), nb_new = ds->NB_after_prune;
+        const unsigned long long new_slots = table_slots_for(p, nb_new);
         phase_prune_move(p, st, ds);
         cl.sync();
-        phase_zero_after_move(p, st, ds);
-        cl.sync();
-        if (gtid() == 0) after_compact(p, ds);
+        {   // one phase instead of three: zero the vacated rows / marks, update the state, clear the
+            // resized table. Everybody works from the snapshot, only thread 0 writes the state.
+            for (uint64_t i = (uint64_t)nb_new * 64 + gtid(); i < (uint64_t)nb_old * 64; i += gthreads()) { st.Q[i] = 0.0; st.Qn[i] = 0.0; }
+            for (uint32_t i = gtid(); i < nb_old; i += gthreads()) st.keep[i] = 0ull;
+            const uint32_t ntiles = (nb_old + SCAN_TILE - 1) / SCAN_TILE + 1;
+            for (uint32_t i = gtid(); i < ntiles; i += gthreads()) st.tile_state[i] = 0ull;
+            const ulonglong2 e = make_ulonglong2(KEY_EMPTY, KEY_EMPTY);
+            for (uint64_t s = gtid(); s < new_slots; s += gthreads()) { st.table[s] = e; st.pend[s] = 0ull; }
+            if (gtid() == 0) after_compact(p, ds);
+        }
         cl.sync();
         st = resolve(st_in, ds);                         // survivors live in the other buffers now
-        phase_clear_table(st, ds);
-        cl.sync();
         phase_rebuild(p, st, ds);
         phase_smax<NDIM, DYN>(p, st, ds);
         phase_sum(p, st, ds, true);
