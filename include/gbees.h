@@ -27,7 +27,7 @@ extern "C" {
 #endif
 
 #define GBEES_OK 0
-#define GBEES_ERR_ARG (-1)        /* bad argument (n out of [1,6], dx <= 0, wrong n_params, NULL) */
+#define GBEES_ERR_ARG (-1)        /* bad argument (n out of [1,6], dx <= 0, threshold <= 0, wrong n_params, NULL) */
 #define GBEES_ERR_CUDA (-2)       /* a CUDA runtime call failed (message in gbees_last_error) */
 #define GBEES_ERR_NOT_SPD (-3)    /* cov / R is not symmetric positive definite */
 #define GBEES_ERR_CAPACITY (-4)   /* more cells than opts.max_cells (fixed capacity) */

@@ -476,6 +476,7 @@ int gbees_create(gbees_ctx** out, int n, const double* dx, double threshold, int
     if (dynamics_id < 0 || dynamics_id > 4 || n_params < need || (need && !params)) return GBEES_ERR_ARG;
     if ((dynamics_id <= 1 && n != 3) || (dynamics_id == 2 && n < 4)) return GBEES_ERR_ARG;
     for (int j = 0; j < n; ++j) if (!(dx[j] > 0.0)) return GBEES_ERR_ARG;
+    if (!(threshold > 0.0)) return GBEES_ERR_ARG;   // p* > 0: a cell with P = 0 must never be a grow source
 
     gbees_ctx* c = new gbees_ctx();
     c->device = o.device;

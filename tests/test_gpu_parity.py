@@ -147,6 +147,9 @@ def test_errors_and_edges():
     with pytest.raises(GbeesError) as e:
         g.step()                                           # empty grid
     assert e.value.code == -6
+    with pytest.raises(GbeesError) as e:
+        G(3, [0.5] * 3, 0.0, 0, [10, 8 / 3, 28])          # threshold must be positive
+    assert e.value.code == -1
     # key range: 6-D fields hold [-512, 511]
     g = G(6, [0.5] * 6, 1e-3, 4, [1.0] * 6, max_cells=4096)
     g.import_state(np.zeros(6), np.array([[511, 0, 0, 0, 0, 0]], dtype=np.int32), np.array([1.0]))
