@@ -33,6 +33,7 @@ def lib():
         L.gbeeso_face_velocity.argtypes = [vp, ip, C.c_int]
         L.gbeeso_face_velocity.restype = C.c_double
         L.gbeeso_targets.argtypes = [vp, ip, ip]
+        L.gbeeso_dynamics.argtypes = [vp, dp, dp]
         L.gbeeso_ht_lookup.argtypes = [C.POINTER(C.c_uint64), C.c_int64, C.POINTER(C.c_uint64),
                                        C.c_int64, C.POINTER(C.c_uint8)]
         _lib = L
@@ -138,6 +139,13 @@ class Oracle:
     def face_velocity(self, coords, j):
         _, c = _i(coords)
         return float(lib().gbeeso_face_velocity(self._h, c, int(j)))
+
+    def dynamics(self, x):
+        """f(x) at an arbitrary point (test hook for the dynamics pins)."""
+        xa, xp = _d(x)
+        out = np.zeros(self.n)
+        lib().gbeeso_dynamics(self._h, xp, out.ctypes.data_as(C.POINTER(C.c_double)))
+        return out
 
     def targets(self, coords):
         _, c = _i(coords)

@@ -18,7 +18,9 @@
 // shift (bit exact), P3 n-D constant-velocity closed form for all sign patterns,
 // P4 1-D binomial smear, P5 Lax-Wendroff, P6 TVD + order, P7 dense-array brute force
 // (oracle/dense_ctu.py, gather form), P8 dt closed form, P9 linear-dynamics moments,
-// P10 Bayes/Kalman, P12 grow/prune duality, P13 reflection.
+// P10 Bayes/Kalman, P12 grow/prune duality, P13 reflection; dynamics() ids 0-4 by what the paper
+// and the mathematics fix (test_D_*: equilibria, "(F, ..., F) is an unstable equilibrium",
+// energy conservation of the Lorenz '96 advection term, divergence, Jacobian structure of PAPER.md:303/319).
 // PARITY UNPINNED against the paper's own software: the limiter family (A3), the exact
 // edge-growth test (A10/A11), the normalisation cadence (A9). See DESIGN.md.
 //
@@ -622,6 +624,14 @@ double gbeeso_face_velocity(void* h, const int32_t* coords, int j) {
     Coord c{};
     for (int m = 0; m < o->n; ++m) c[m] = coords[m];
     return face_velocity(*o, c, j);
+}
+
+// test hook for the dynamics pins (tests/test_oracle_pins.py): out[j] = f_j(x) at an arbitrary point x,
+// through the same dynamics() the face velocities use
+int gbeeso_dynamics(void* h, const double* x, double* out) {
+    Oracle* o = (Oracle*)h;
+    for (int j = 0; j < o->n; ++j) out[j] = dynamics(*o, x, j);
+    return 0;
 }
 
 // number of grow targets of cell `coords` and (optionally) their coordinates [<= 72 * n]

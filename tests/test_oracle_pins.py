@@ -37,12 +37,22 @@ def test_P1_conservation_when_support_is_two_cells_inside(n, dyn, params):
     keys = box([0] * n, [side] * n)
     inner = np.all((keys >= 2) & (keys < side - 2), axis=1)
     p = np.where(inner, rng.random(len(keys)), 0.0)
-    # ragged: drop a random 30% of the zero cells that are not within 2 cells of the support
-    o = raw(n, [0.5] * n, dyn, params, keys, p, origin=[1.0] * n)
-    o.step()
-    _, p1 = o.export()
-    assert abs(p1.sum() - p.sum()) <= len(keys) * 2.0 ** -52 * p.sum()
-    assert abs(o.last_mass() - p.sum()) <= len(keys) * 2.0 ** -52 * p.sum()
+    for ragged in (False, True):
+        k2, p2 = keys, p
+        if ragged:
+            # ragged active set: with d = sum_j (distance of coordinate j outside the support's box), a random
+            # 30 % of the zero cells with d >= 3 are dropped. Cells that then miss a face neighbour have
+            # d >= 2, so they and all their face neighbours (d >= 1) carry no mass: P1's premise holds.
+            d = np.sum(np.maximum(2 - keys, 0) + np.maximum(keys - (side - 3), 0), axis=1)
+            drop = (d >= 3) & (rng.random(len(keys)) < 0.3)
+            assert drop.sum() > 0
+            k2, p2 = keys[~drop], p2[~drop]
+        o = raw(n, [0.5] * n, dyn, params, k2, p2, origin=[1.0] * n)
+        o.step()
+        _, p1 = o.export()
+        assert len(p1) == len(p2)
+        assert abs(p1.sum() - p2.sum()) <= len(k2) * 2.0 ** -52 * p2.sum()
+        assert abs(o.last_mass() - p2.sum()) <= len(k2) * 2.0 ** -52 * p2.sum()
 
 
 def test_P1_mass_is_lost_only_through_boundary_faces():
@@ -259,6 +269,119 @@ def test_A12_face_velocity_matches_independent_numpy():
                 x = [np.float64(origin[m] + (c[m] - (0.5 if m == j else 0.0)) * h[m]) for m in range(n)]
                 want = float(dense_ctu.dynamics(dyn, params, x, j))
                 assert o.face_velocity(c, j) == pytest.approx(want, rel=1e-13, abs=1e-13)
+
+
+# ---- dynamics pins: what the paper and the mathematics fix about f(x), with no second typing of f ------
+def _oracle_for(n, dyn, params):
+    return raw(n, [0.5] * n, dyn, params, np.zeros((1, n), dtype=np.int32), [1.0])
+
+
+def _jacobian(o, x, eps=0.5):
+    """Central differences; exact up to rounding for the (at most quadratic) Lorenz fields."""
+    n = len(x)
+    J = np.zeros((n, n))
+    for m in range(n):
+        e = np.zeros(n); e[m] = eps
+        J[:, m] = (o.dynamics(x + e) - o.dynamics(x - e)) / (2 * eps)
+    return J
+
+
+@pytest.mark.parametrize("n", [4, 5, 6])
+def test_D_lorenz96_equilibrium_energy_divergence(n):
+    # PAPER.md:319: f_j = (x_{j+1} - x_{j-2}) x_{j-1} - x_j + F, cyclic; "(F, ..., F) is an unstable equilibrium"
+    F = 4.0
+    o = _oracle_for(n, 2, [F])
+    assert np.array_equal(o.dynamics(np.full(n, F)), np.zeros(n))          # exactly: (F - F) F - F + F
+    rng = np.random.default_rng(S0 + 300 + n)
+    for _ in range(20):
+        x = rng.normal(0, 3, n)
+        f = o.dynamics(x)
+        # the quadratic (advection) term conserves energy: sum_j x_j (x_{j+1} - x_{j-2}) x_{j-1} = 0.
+        # Any wrong cyclic index (x_{j+2} for x_{j-2}, x_{j+1} for x_{j-1}, ...) breaks the cancellation.
+        quad = f + x - F
+        assert abs(np.dot(x, quad)) <= 1e-12 * np.sum(np.abs(x) ** 3 + 1)
+        J = _jacobian(o, x)
+        assert np.allclose(np.diag(J), -1.0, atol=1e-12)                   # div f = -n
+        # Jacobian structure of the printed formula: df_j/dx_{j+1} = x_{j-1}, df_j/dx_{j-2} = -x_{j-1},
+        # df_j/dx_{j-1} = x_{j+1} - x_{j-2}; everything else 0
+        for j in range(n):
+            want = np.zeros(n)
+            want[j] += -1.0
+            want[(j + 1) % n] += x[(j - 1) % n]
+            want[(j - 2) % n] += -x[(j - 1) % n]
+            want[(j - 1) % n] += x[(j + 1) % n] - x[(j - 2) % n]
+            assert np.allclose(J[j], want, atol=1e-11), (j, J[j], want)
+    # instability of (F,...,F): the Jacobian there has an eigenvalue with positive real part (n = 6, F = 4)
+    if n == 6:
+        assert np.max(np.linalg.eigvals(_jacobian(o, np.full(n, F))).real) > 0.1
+
+
+def test_D_lorenz63_classic_fixed_points_divergence_symmetry():
+    # BASELINE.json configs[0-1]: classic Lorenz '63, (sigma, beta, rho) = (10, 8/3, 28)
+    s_, b_, r_ = 10.0, 8.0 / 3.0, 28.0
+    o = _oracle_for(3, 0, [s_, b_, r_])
+    q = math.sqrt(b_ * (r_ - 1.0))
+    assert np.array_equal(o.dynamics(np.zeros(3)), np.zeros(3))
+    for sgn in (1.0, -1.0):
+        assert np.allclose(o.dynamics(np.array([sgn * q, sgn * q, r_ - 1.0])), 0.0, atol=1e-12)
+    rng = np.random.default_rng(S0 + 310)
+    for _ in range(10):
+        x = rng.normal(0, 10, 3)
+        J = _jacobian(o, x)
+        assert np.trace(J) == pytest.approx(-(s_ + 1.0 + b_), abs=1e-10)    # div f = -(sigma + 1 + beta)
+        want = np.array([[-s_, s_, 0.0], [r_ - x[2], -1.0, -x[0]], [x[1], x[0], -b_]])
+        assert np.allclose(J, want, atol=1e-9)
+        # symmetry (x1, x2, x3) -> (-x1, -x2, x3)
+        f, g = o.dynamics(x), o.dynamics(x * np.array([-1.0, -1.0, 1.0]))
+        assert np.allclose(g, f * np.array([-1.0, -1.0, 1.0]), atol=1e-12)
+
+
+def test_D_lorenz63_paper_form_fixed_points_divergence():
+    # PAPER.md:303: f = (sigma (x2 - x1), -x2 - x1 x3, -b x3 + x1 x2 - b r), (sigma, b, r) = (4, 1, 48)
+    s_, b_, r_ = 4.0, 1.0, 48.0
+    o = _oracle_for(3, 1, [s_, b_, r_])
+    # fixed points: x1 = x2; x2 (1 + x3) = 0 -> (0, 0, -r) and x3 = -1, x1^2 = b (r - 1)
+    assert np.allclose(o.dynamics(np.array([0.0, 0.0, -r_])), 0.0, atol=1e-13)
+    q = math.sqrt(b_ * (r_ - 1.0))
+    for sgn in (1.0, -1.0):
+        assert np.allclose(o.dynamics(np.array([sgn * q, sgn * q, -1.0])), 0.0, atol=1e-12)
+    assert np.allclose(o.dynamics(np.zeros(3)), [0.0, 0.0, -b_ * r_])
+    rng = np.random.default_rng(S0 + 311)
+    for _ in range(10):
+        x = rng.normal(0, 10, 3)
+        J = _jacobian(o, x)
+        assert np.trace(J) == pytest.approx(-(s_ + 1.0 + b_), abs=1e-10)
+        want = np.array([[-s_, s_, 0.0], [-x[2], -1.0, -x[0]], [x[1], x[0], -b_]])
+        assert np.allclose(J, want, atol=1e-9)
+    # it is the classic system with z shifted by r: f_paper(x1, x2, x3) = f_classic(x1, x2, x3 + r)
+    oc = _oracle_for(3, 0, [s_, b_, r_])
+    x = rng.normal(0, 5, 3)
+    assert np.allclose(o.dynamics(x), oc.dynamics(x + np.array([0.0, 0.0, r_])), atol=1e-10)
+
+
+def test_D_linear_and_constant_dynamics_are_what_they_say():
+    rng = np.random.default_rng(S0 + 312)
+    A = rng.normal(0, 0.3, (5, 5))
+    o = _oracle_for(5, 3, A.ravel())
+    x = rng.normal(0, 2, 5)
+    assert np.allclose(_jacobian(o, x), A, atol=1e-12)                      # f = A x: Jacobian is A (row-major)
+    assert np.array_equal(o.dynamics(np.zeros(5)), np.zeros(5))
+    v = rng.normal(0, 1, 4)
+    oc = _oracle_for(4, 4, v)
+    assert np.array_equal(oc.dynamics(rng.normal(0, 1, 4)), v)
+
+
+def test_D_face_velocity_is_the_dynamics_at_the_lower_face_centre():
+    # Eq. (7) text, PAPER.md:82: the flux velocity is f_j at the centre of face i - e^j / 2
+    rng = np.random.default_rng(S0 + 313)
+    n, h, origin = 6, rng.uniform(0.2, 0.6, 6), rng.normal(0, 3, 6)
+    o = raw(n, h, 2, [4.0], np.zeros((1, n), dtype=np.int32), [1.0], origin=origin)
+    for _ in range(10):
+        c = rng.integers(-30, 30, n).astype(np.int32)
+        for j in range(n):
+            x = origin + c * h
+            x[j] = origin[j] + (c[j] - 0.5) * h[j]
+            assert o.face_velocity(c, j) == o.dynamics(x)[j]
 
 
 # ---- P9 linear dynamics: grid moments follow N(e^{At} mu, e^{At} Sigma e^{A^T t}) ---------------------
