@@ -163,10 +163,6 @@ int gbees_stats(gbees_ctx* ctx, gbees_stats_t* out /*host*/);
  * Launch counts are always kept; milliseconds only while profiling is enabled. While profiling is on
  * gbees_run always uses the per-phase launches (never the single-launch loop for small grids). */
 int gbees_profile(gbees_ctx* ctx, int enable, double* phase_ms, int64_t* phase_launches);
-/* Kept for ABI stability: per-phase device timers of the former persistent kernel. The phases of
- * gbees_run are separate launches now and are timed by gbees_profile; this call returns zeros.
- * phase_ms: host [GBEES_PHASES]. */
-int gbees_run_breakdown(gbees_ctx* ctx, double* phase_ms);
 const char* gbees_last_error(gbees_ctx* ctx);
 int gbees_clear_error(gbees_ctx* ctx);
 

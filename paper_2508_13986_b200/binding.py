@@ -63,7 +63,6 @@ def lib():
         L.gbees_marginal.argtypes = [vp, C.POINTER(C.c_int), C.c_int, vp, vp, C.c_int64, C.POINTER(C.c_int64)]
         L.gbees_stats.argtypes = [vp, C.POINTER(Stats)]
         L.gbees_profile.argtypes = [vp, C.c_int, dp, C.POINTER(C.c_int64)]
-        L.gbees_run_breakdown.argtypes = [vp, dp]
         L.gbees_last_error.argtypes = [vp]
         L.gbees_last_error.restype = C.c_char_p
         L.gbees_clear_error.argtypes = [vp]
@@ -197,12 +196,6 @@ class Gbees:
         ln = (C.c_int64 * len(PHASES))()
         self._chk(lib().gbees_profile(self._h, int(bool(enable)), ms, ln))
         return {k: (ms[i], ln[i]) for i, k in enumerate(PHASES)}
-
-    def run_breakdown(self):
-        """Read-and-reset {phase: ms} spent inside the persistent kernel (device timer)."""
-        ms = (C.c_double * len(PHASES))()
-        self._chk(lib().gbees_run_breakdown(self._h, ms))
-        return {k: ms[i] for i, k in enumerate(PHASES) if ms[i] > 0}
 
     def last_mass(self):
         return self.stats()["mass"]

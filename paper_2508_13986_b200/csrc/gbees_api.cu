@@ -133,7 +133,9 @@ __global__ void __launch_bounds__(TPB) k_run_small(GP, int prune_every, int no_g
     unsigned long long k = k_start;
     for (;;) {
         cl.sync();
-        if (!ds->go || ds->NB > nb_limit) break;        // uniform: nothing writes these before the next barrier
+        // uniform: go and NB_before_grow (= NB at the top of the loop) are written by begin_step only, i.e.
+        // before this barrier; NB itself is bumped by the grow below and must not be tested here
+        if (!ds->go || ds->NB_before_grow > nb_limit) break;
         Store st = resolve(st_in, ds);
         if (!no_grow) {
             phase_targets<NDIM, DYN, true>(p, st, ds);
@@ -267,8 +269,6 @@ struct gbees_ctx {
     std::vector<cudaEvent_t> ev_free;
     std::vector<std::pair<int, std::pair<cudaEvent_t, cudaEvent_t>>> ev_open;
     double phase_ms[GBEES_PHASES] = {0};
-    double run_phase_ms[GBEES_PHASES] = {0};   // breakdown inside the persistent kernel (device timer)
-    int run_ns_dirty = 0;
     int64_t phase_launches[GBEES_PHASES] = {0};
 };
 
@@ -371,17 +371,6 @@ int sync_state(gbees_ctx* c) {
     CU(cudaMemcpyAsync(c->h_st, c->d_st, sizeof(DevState), cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
     if (c->profile) drain_events(c);
-    // persistent loop: fold the device-timer phase breakdown into the accumulators
-    for (int k = 0; k < GBEES_PH_RUN; ++k)
-        if (c->h_st->phase_ns[k]) {
-            c->run_phase_ms[k] += 1e-6 * (double)c->h_st->phase_ns[k];
-            c->h_st->phase_ns[k] = 0;
-            c->run_ns_dirty = 1;
-        }
-    if (c->run_ns_dirty) {
-        cudaMemsetAsync(c->d_st->phase_ns, 0, sizeof(c->h_st->phase_ns), c->stream);
-        c->run_ns_dirty = 0;
-    }
     const int e = c->h_st->err;
     if (e & E_CAPACITY) return fail(c, GBEES_ERR_CAPACITY, "cell pool capacity (opts.max_cells) exceeded");
     if (e & E_TABLE_FULL) return fail(c, GBEES_ERR_CAPACITY, "hashtable full");
@@ -471,7 +460,7 @@ int gbees_create(gbees_ctx** out, int n, const double* dx, double threshold, int
     if (o.max_cells <= 0) o.max_cells = 1 << 20;
     if (!(o.load_factor > 0.0 && o.load_factor < 1.0)) o.load_factor = 0.5;
     if (!(o.cfl > 0.0)) o.cfl = 0.9;
-    if (o.max_cells >= (int64_t)1 << 36) return GBEES_ERR_ARG;   // brick rows are 32-bit
+    if (o.max_cells >= (int64_t)1 << 32) return GBEES_ERR_ARG;   // export / marginal row counters are 32-bit
     const int need = dynamics_id == 0 || dynamics_id == 1 ? 3 : dynamics_id == 2 ? 1 : dynamics_id == 3 ? n * n : n;
     if (dynamics_id < 0 || dynamics_id > 4 || n_params < need || (need && !params)) return GBEES_ERR_ARG;
     if ((dynamics_id <= 1 && n != 3) || (dynamics_id == 2 && n < 4)) return GBEES_ERR_ARG;
@@ -516,6 +505,16 @@ int gbees_create(gbees_ctx** out, int n, const double* dx, double threshold, int
     c->grid = (unsigned)c->sms * 8u;
     c->grid_flux1 = (unsigned)c->sms * 2u;     // = resident blocks at 128 registers: a persistent grid-stride grid (measured best of 2/4/8/16)
     c->ntiles_max = (p.capB + SCAN_TILE - 1) / SCAN_TILE;
+    // dynamic shared memory above 48 KB is an opt-in per function AND per device: set it for this context's device
+    if (dispatch(c, [&](auto N_, auto D_) {
+            constexpr int NN = decltype(N_)::value, DD = decltype(D_)::value;
+            constexpr int smem = (int)(sizeof(Flux1Smem<NN>) * WPB);
+            if (cudaFuncSetAttribute(k_flux1<NN, DD, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess ||
+                cudaFuncSetAttribute(k_flux1<NN, DD, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
+                return GBEES_ERR_CUDA;
+            return GBEES_OK;
+        }) != GBEES_OK)
+        return bail(GBEES_ERR_CUDA, "unsupported (n, dynamics) pair or shared-memory opt-in failed");
     const size_t cb = p.capB, nd = 2 * (size_t)n;
     auto alloc = [&](void** ptr, size_t bytes) {
         cudaError_t e2 = cudaMalloc(ptr, bytes);
@@ -633,13 +632,7 @@ static int enqueue_step(gbees_ctx* c) {
             phase(c, GBEES_PH_LINK, 1, [&] { k_link<NN, false><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 1); });
         }
         phase(c, GBEES_PH_PASSA, 1, [&] {
-            constexpr size_t smem = sizeof(Flux1Smem<NN>) * WPB;
-            static bool attr_set = false;
-            if (!attr_set) {
-                cudaFuncSetAttribute(k_flux1<NN, DD, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-                cudaFuncSetAttribute(k_flux1<NN, DD, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-                attr_set = true;
-            }
+            constexpr size_t smem = sizeof(Flux1Smem<NN>) * WPB;   // opt-in above 48 KB: set per device in gbees_create
             if (c->p.hi_res && !c->p.limiter) k_flux1<NN, DD, true><<<c->grid_flux1, TPB, smem, c->stream>>>(c->p, c->st, c->d_st);
             else k_flux1<NN, DD, false><<<c->grid_flux1, TPB, smem, c->stream>>>(c->p, c->st, c->d_st);
         });
@@ -797,7 +790,7 @@ int gbees_compare(gbees_ctx* c, gbees_ctx* o, double* bc, double* l1) {
     dispatch_n(c, [&](auto N_) {
         k_compare<decltype(N_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, o->st, o->d_st, part);
         k_compare_finish<<<1, TPB, 0, c->stream>>>(part, c->grid, res);
-        k_compare<decltype(N_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, o->st, o->d_st, c->st, c->d_st, part);
+        k_compare<decltype(N_)::value><<<c->grid, TPB, 0, c->stream>>>(o->p, o->st, o->d_st, c->st, c->d_st, part);   // the scanned side's own capB
         k_compare_finish<<<1, TPB, 0, c->stream>>>(part, c->grid, res + 3);
         return GBEES_OK;
     });
@@ -831,7 +824,7 @@ int gbees_marginal(gbees_ctx* c, const int* dims, int m, int32_t* keys, double* 
     while (g.S < 2 * N) g.S <<= 1;                                // at most N marginal cells: load factor <= 0.5
     // scratch in the phi array (free between steps): table keys, table values, then the output staging area
     const size_t need = (size_t)g.S * 16 + (size_t)N * (4 * (size_t)m + 8) + 64;
-    if (need > c->stage_bytes) return fail(c, GBEES_ERR_CAPACITY, "marginal: scratch larger than the staging area");
+    if (need > c->stage_bytes) { c->err = "marginal: scratch larger than the staging area"; return GBEES_ERR_CAPACITY; }   // a query: not sticky
     unsigned long long* skey = reinterpret_cast<unsigned long long*>(c->st.phi);
     double* sval = reinterpret_cast<double*>(skey + g.S);
     char* stage = reinterpret_cast<char*>(sval + g.S);
@@ -1017,12 +1010,6 @@ int gbees_stats(gbees_ctx* c, gbees_stats_t* s) {
     s->cells_inserted = (int64_t)c->h_st->inserted_total;
     s->cells_prune_scanned = (int64_t)c->h_st->prune_scanned;
     s->prunes = (int64_t)c->h_st->prunes;
-    return GBEES_OK;
-}
-
-int gbees_run_breakdown(gbees_ctx* c, double* phase_ms) {
-    if (!c || !phase_ms) return GBEES_ERR_ARG;
-    for (int k = 0; k < GBEES_PHASES; ++k) { phase_ms[k] = c->run_phase_ms[k]; c->run_phase_ms[k] = 0.0; }
     return GBEES_OK;
 }
 

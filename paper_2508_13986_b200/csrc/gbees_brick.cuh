@@ -135,9 +135,10 @@ __device__ void phase_targets(const Params& p, const Store& st, DevState* ds) {
     __shared__ unsigned long long sTb[WPB][ND + 1];   // merged target bits per destination (face neighbours, own)
     __shared__ uint8_t sItem[WPB][NT + 1];            // work list of the non-empty destinations / diagonal classes
     __shared__ unsigned long long sEdge[ND];
-    __shared__ unsigned long long sQk[GROW ? WPB : 1][GROW ? NT : 1], sQm[GROW ? WPB : 1][GROW ? NT : 1];   // new cells: (brick key, bits)
+    // new cells: (brick key, bits); one entry per work item at most (own brick + 2n faces + NT - 2n diagonal classes)
+    __shared__ unsigned long long sQk[GROW ? WPB : 1][GROW ? NT + 1 : 1], sQm[GROW ? WPB : 1][GROW ? NT + 1 : 1];
     __shared__ unsigned sQn[WPB];
-    __shared__ unsigned sQo[GROW ? WPB : 1][GROW ? NT : 1];   // exclusive prefix of the new-cell counts
+    __shared__ unsigned sQo[GROW ? WPB : 1][GROW ? NT + 1 : 1];   // exclusive prefix of the new-cell counts
     if (threadIdx.x < ND) sEdge[threadIdx.x] = edge_mask<NDIM>(threadIdx.x >> 1, threadIdx.x & 1);
     __syncthreads();
     const uint32_t NB0 = GROW ? ds->NB_before_grow : min(ds->NB, p.capB);
@@ -485,7 +486,6 @@ __device__ void phase_flux1(const Params& p, const Store& st, DevState* ds) {
                 face_velocities<NDIM, DYN>(p, c, ul, uu);
 #pragma unroll
                 for (int j = 0; j < NDIM; ++j) {
-                    constexpr int dummy = 0; (void)dummy;
                     const int s = 1 << G::SH(j), MK = G::MK(j);
                     const int lj = (l >> G::SH(j)) & MK;
                     const int im = lj > 0 ? OWN * 64 + l - s : (2 * j) * 64 + l + MK * s;

@@ -62,7 +62,6 @@ struct DevState {
     unsigned long long step_limit;       // ... or until steps == step_limit
     int go;                              // the step being enqueued executes (decided on the device by begin_step)
     int prune_ok;                        // the last enqueued step executed: the prune that follows it runs
-    unsigned long long phase_ns[12];     // persistent loop: device-timer ns per phase (index = GBEES_PH_*)
     unsigned long long slots;            // hashtable slots in use (<= Params::slots), resized at rehash
 };
 
@@ -253,7 +252,6 @@ __device__ __forceinline__ void cfl_fold(const Params& p, const double ul[NDIM],
     if (sa >= best * (1.0 - 1e-12)) best = fmax(best, cfl_term<NDIM>(p, ul));
 }
 
-// monotonised-central limiter, division-free (A3)
 // active table size for NB bricks: room for the brick count to grow 8x before the load factor is
 // reached, never below 2^16 slots, never above the allocation
 __host__ __device__ __forceinline__ unsigned long long table_slots_for(const Params& p, unsigned long long NB) {
@@ -262,6 +260,7 @@ __host__ __device__ __forceinline__ unsigned long long table_slots_for(const Par
     return want < p.slots ? want : p.slots;
 }
 
+// monotonised-central limiter, division-free (A3)
 __device__ __forceinline__ double mc_limit(double a, double b) {
     if (a * b <= 0.0) return 0.0;
     const double m = fmin(0.5 * fabs(a + b), fmin(2.0 * fabs(a), 2.0 * fabs(b)));

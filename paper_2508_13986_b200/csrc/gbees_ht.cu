@@ -137,17 +137,23 @@ int gbees_ht_create(gbees_ht** out, int64_t slots, int device) {
     gbees_ht* h = new gbees_ht();
     h->device = device;
     h->slots = (uint64_t)slots;
-    HT_CU(cudaSetDevice(device));
-    cudaDeviceProp prop;
-    HT_CU(cudaGetDeviceProperties(&prop, device));
-    h->grid = (unsigned)prop.multiProcessorCount * 8u;
-    HT_CU(cudaMalloc((void**)&h->table, h->slots * sizeof(ulonglong2)));
-    HT_CU(cudaMalloc((void**)&h->count, 4));
-    HT_CU(cudaMalloc((void**)&h->probes, 8));
-    HT_CU(cudaMalloc((void**)&h->tile_counter, 4));
-    HT_CU(cudaMalloc((void**)&h->total, 4));
-    HT_CU(cudaMemset(h->table, 0xFF, h->slots * sizeof(ulonglong2)));
-    HT_CU(cudaMemset(h->count, 0, 4));
+    // on any failure the handle and whatever was allocated so far are released
+    auto build = [&]() -> int {
+        HT_CU(cudaSetDevice(device));
+        cudaDeviceProp prop;
+        HT_CU(cudaGetDeviceProperties(&prop, device));
+        h->grid = (unsigned)prop.multiProcessorCount * 8u;
+        HT_CU(cudaMalloc((void**)&h->table, h->slots * sizeof(ulonglong2)));
+        HT_CU(cudaMalloc((void**)&h->count, 4));
+        HT_CU(cudaMalloc((void**)&h->probes, 8));
+        HT_CU(cudaMalloc((void**)&h->tile_counter, 4));
+        HT_CU(cudaMalloc((void**)&h->total, 4));
+        HT_CU(cudaMemset(h->table, 0xFF, h->slots * sizeof(ulonglong2)));
+        HT_CU(cudaMemset(h->count, 0, 4));
+        return GBEES_OK;
+    };
+    const int rc = build();
+    if (rc != GBEES_OK) { gbees_ht_destroy(h); return rc; }
     *out = h;
     return GBEES_OK;
 }
