@@ -38,6 +38,7 @@ __global__ void k_begin_run(DevState* ds, double t_target, unsigned long long st
     begin_step(ds);
 }
 __global__ void k_set_prune_ok(DevState* ds) { ds->prune_ok = 1; }
+__global__ void __launch_bounds__(TPB) k_detect(GP) { GUARD(1); ST; phase_detect(p, st, ds); }
 template <int NDIM, int DYN>
 __global__ void __launch_bounds__(TPB) k_grow(GP) { GUARD(1); ST; phase_targets<NDIM, DYN, true>(p, st, ds); }
 template <int NDIM, int DYN>
@@ -138,6 +139,8 @@ __global__ void __launch_bounds__(TPB) k_run_small(GP, int prune_every, int no_g
         if (!ds->go || ds->NB_before_grow > nb_limit) break;
         Store st = resolve(st_in, ds);
         if (!no_grow) {
+            phase_detect(p, st, ds);
+            cl.sync();
             phase_targets<NDIM, DYN, true>(p, st, ds);
             cl.sync();
             phase_link<NDIM, false>(p, st, ds);
@@ -319,18 +322,24 @@ template <typename F>
 int dispatch(const gbees_ctx* c, F&& f) {
     const int n = c->p.n, d = c->p.dyn;
 #define GB_CASE(N_, D_) if (n == N_ && d == D_) return f(IC<N_>{}, IC<D_>{});
+#ifdef GBEES_DEV_PAIRS   // development builds: only the benchmarked pairs (seconds instead of minutes to compile)
+    GB_CASE(3, 0) GB_CASE(6, 2) GB_CASE(6, 3)
+#else
     GB_CASE(3, 0) GB_CASE(3, 1)
     GB_CASE(4, 2) GB_CASE(5, 2) GB_CASE(6, 2)
     GB_CASE(1, 3) GB_CASE(2, 3) GB_CASE(3, 3) GB_CASE(4, 3) GB_CASE(5, 3) GB_CASE(6, 3)
     GB_CASE(1, 4) GB_CASE(2, 4) GB_CASE(3, 4) GB_CASE(4, 4) GB_CASE(5, 4) GB_CASE(6, 4)
+#endif
 #undef GB_CASE
     return GBEES_ERR_ARG;
 }
 template <typename F>
 int dispatch_n(const gbees_ctx* c, F&& f) {
     switch (c->p.n) {
-        case 1: return f(IC<1>{}); case 2: return f(IC<2>{}); case 3: return f(IC<3>{});
-        case 4: return f(IC<4>{}); case 5: return f(IC<5>{}); case 6: return f(IC<6>{});
+#ifndef GBEES_DEV_PAIRS
+        case 1: return f(IC<1>{}); case 2: return f(IC<2>{}); case 4: return f(IC<4>{}); case 5: return f(IC<5>{});
+#endif
+        case 3: return f(IC<3>{}); case 6: return f(IC<6>{});
     }
     return GBEES_ERR_ARG;
 }
@@ -526,7 +535,7 @@ int gbees_create(gbees_ctx** out, int n, const double* dx, double threshold, int
     if (alloc((void**)&st.Q, cb * 512) || alloc((void**)&st.Qn, cb * 512) || alloc((void**)&st.phi, c->stage_bytes) ||
         alloc((void**)&st.bkey, cb * 8) || alloc((void**)&st.mask, cb * 8) || alloc((void**)&st.grown, cb * 8) ||
         alloc((void**)&st.keep, cb * 8) || alloc((void**)&st.fetch, cb * 64 * 2) || alloc((void**)&st.adj, cb * nd * 4) ||
-        alloc((void**)&st.slot_of, cb * 4) || alloc((void**)&st.table, p.slots * sizeof(ulonglong2)) ||
+        alloc((void**)&st.slot_of, cb * 4) || alloc((void**)&st.slist, cb * 4) || alloc((void**)&st.smask, cb * 8) || alloc((void**)&st.table, p.slots * sizeof(ulonglong2)) ||
         alloc((void**)&st.pend, p.slots * 8) || alloc((void**)&st.bkey2, cb * 8) || alloc((void**)&st.mask2, cb * 8) ||
         alloc((void**)&st.grown2, cb * 8) || alloc((void**)&st.newrow, cb * 4) ||
         alloc((void**)&st.tile_state, (size_t)(c->ntiles_max + 1) * 8) || alloc((void**)&st.partial, (size_t)c->grid * 8) ||
@@ -628,7 +637,10 @@ static int enqueue_step(gbees_ctx* c) {
     int rc = dispatch(c, [&](auto N_, auto D_) {
         constexpr int NN = decltype(N_)::value, DD = decltype(D_)::value;
         if (!c->no_grow) {
-            phase(c, GBEES_PH_GROW, 1, [&] { k_grow<NN, DD><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st); });
+            phase(c, GBEES_PH_GROW, 2, [&] {
+                k_detect<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
+                k_grow<NN, DD><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
+            });
             phase(c, GBEES_PH_LINK, 1, [&] { k_link<NN, false><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 1); });
         }
         phase(c, GBEES_PH_PASSA, 1, [&] {

@@ -98,17 +98,18 @@ __device__ __forceinline__ unsigned long long edge_mask(int j, int side) {   // 
 }
 
 // GROW: activate the cells `bits` of the brick in row `row` (NBR_NONE: unknown, look `key` up and
-// create it if absent). Returns the bits this thread switched on; `key` then holds the brick's key.
-__device__ __forceinline__ unsigned long long grow_apply(const Params& p, const Store& st, DevState* ds, uint32_t NB0,
-                                                         uint64_t slots, int nd, uint32_t row, uint64_t key,
-                                                         unsigned long long bits) {
+// create it if absent). Nothing is returned: the atomics are fire-and-forget (RED), so a source brick
+// never waits for them; which cells were new is not needed (the CFL terms are folded for every
+// target, the maximum is idempotent, and pass 1 recounts the active cells).
+__device__ __forceinline__ void grow_apply(const Params& p, const Store& st, DevState* ds, uint32_t NB0,
+                                           uint64_t slots, int nd, uint32_t row, uint64_t key, unsigned long long bits) {
     if (row == NBR_NONE) {
         bool inserted;
         const uint64_t s = ht_upsert(st.table, slots, key, inserted);
-        if (s == ~0ull) { atomicOr(&ds->err, E_TABLE_FULL); return 0ull; }
+        if (s == ~0ull) { atomicOr(&ds->err, E_TABLE_FULL); return; }
         if (inserted) {
             const uint32_t nr = atomicAdd(&ds->NB, 1u);
-            if (nr >= p.capB) { atomicOr(&ds->err, E_CAPACITY); return 0ull; }
+            if (nr >= p.capB) { atomicOr(&ds->err, E_CAPACITY); return; }
             st.bkey[nr] = key; st.slot_of[nr] = (uint32_t)s; st.grown[nr] = 0ull; st.mask[nr] = 0ull;
             for (int d = 0; d < nd; ++d) st.adj[(size_t)nr * nd + d] = NBR_NONE;
             __threadfence();
@@ -118,11 +119,31 @@ __device__ __forceinline__ unsigned long long grow_apply(const Params& p, const 
             if (er != NBR_NONE && er < NB0) row = er;       // existed before this launch (diagonal without adjacency)
         }
         // a brick created during this launch collects its bits in pend[slot] (folded in by link)
-        if (row == NBR_NONE) return bits & ~atomicOr((unsigned long long*)&st.pend[s], bits);
+        if (row == NBR_NONE) { atomicOr((unsigned long long*)&st.pend[s], bits); return; }
     }
-    const unsigned long long want = bits & ~*reinterpret_cast<volatile unsigned long long*>(&st.mask[row]);
-    if (!want) return 0ull;
-    return want & ~atomicOr((unsigned long long*)&st.mask[row], want);
+    atomicOr((unsigned long long*)&st.mask[row], bits);
+}
+
+// a1, first half: list the bricks that hold NEW sources (active, P >= p*, targets not inserted yet) with
+// their source masks. The expensive half (phase_targets) then runs over that list, evenly spread over the
+// warps; here a brick costs two dependent loads. A cell grows once (autonomous f): its GROWN bit is set here.
+__device__ inline void phase_detect(const Params& p, const Store& st, DevState* ds) {
+    const uint32_t NB0 = ds->NB_before_grow;
+    const double scale = ds->scale;
+    const unsigned lane = lane_id();
+    for (uint32_t b = gwarp(); b < NB0; b += gwarps()) {   // warp-uniform
+        const uint64_t m = st.mask[b], g = st.grown[b];
+        const uint64_t cand = m & ~g;
+        if (!cand) continue;
+        const bool s0 = ((cand >> lane) & 1ull) && scale * st.Q[(size_t)b * 64 + lane] >= p.thresh;
+        const bool s1 = ((cand >> (lane + 32)) & 1ull) && scale * st.Q[(size_t)b * 64 + 32 + lane] >= p.thresh;
+        const uint64_t src = (uint64_t)__ballot_sync(0xffffffffu, s0) | ((uint64_t)__ballot_sync(0xffffffffu, s1) << 32);
+        if (!src || lane != 0) continue;
+        const uint32_t i = atomicAdd(&ds->nsrc, 1u);
+        st.slist[i] = b;
+        st.smask[i] = src;
+        st.grown[b] = g | src;
+    }
 }
 
 template <int NDIM, int DYN, bool GROW>
@@ -146,22 +167,24 @@ __device__ void phase_targets(const Params& p, const Store& st, DevState* ds) {
     const uint64_t slots = ds->slots;
     const int32_t lo = (int32_t)(-p.bias), hi = (int32_t)(p.bias - 1);
     const unsigned w = threadIdx.x >> 5, lane = lane_id();
-    unsigned long long n_new = 0;
-    const double smax0 = GROW ? __longlong_as_double((long long)ds->smax_bits) : 0.0;   // the maximum so far: most new cells stay below it
+    const double smax0 = GROW ? __longlong_as_double((long long)ds->smax_bits) : 0.0;   // the maximum so far: most target cells stay below it
     double smax = smax0;
-    // new cells (GROW) are queued per warp as (brick key, bits) and expanded by all lanes below
-    auto account = [&](uint64_t key, unsigned long long fresh) {
-        if (!fresh) return;
+    // target cells (GROW) are queued per warp as (brick key, bits) and expanded by all lanes below
+    auto account = [&](uint64_t key, unsigned long long bits) {
         const unsigned k = atomicAdd(&sQn[GROW ? w : 0], 1u);
         sQk[GROW ? w : 0][GROW ? k : 0] = key;
-        sQm[GROW ? w : 0][GROW ? k : 0] = fresh;
+        sQm[GROW ? w : 0][GROW ? k : 0] = bits;
     };
-    for (uint32_t b = gwarp(); b < NB0; b += gwarps()) {   // warp-uniform
+    // GROW: the bricks that hold new sources were listed by phase_detect, so every warp gets the same share of
+    // the expensive bricks; mark: all bricks, sources = every cell with P >= p*.
+    const uint32_t nwork = GROW ? min(ds->nsrc, p.capB) : NB0;
+    for (uint32_t wi = gwarp(); wi < nwork; wi += gwarps()) {   // warp-uniform
+        const uint32_t b = GROW ? st.slist[wi] : wi;
         const uint64_t m = st.mask[b];
-        const uint64_t g = GROW ? st.grown[b] : 0ull;
-        const uint64_t cand = m & ~g;
-        if (!cand) continue;
         const uint64_t bk = st.bkey[b];
+        const uint32_t my_adj = lane < ND ? st.adj[(size_t)b * ND + lane] : NBR_NONE;
+        const uint64_t cand = GROW ? st.smask[wi] : m;        // GROW: the sources themselves
+        if (!cand) continue;
         int32_t B[NDIM];
         unpack<NDIM>(p, bk, B);
         unsigned fl[2] = {0u, 0u};
@@ -170,7 +193,7 @@ __device__ void phase_targets(const Params& p, const Store& st, DevState* ds) {
         for (int hh = 0; hh < 2; ++hh) {
             const int l = (int)lane + 32 * hh;
             bool is_src = false;
-            if ((cand >> l) & 1ull) is_src = scale * st.Q[(size_t)b * 64 + l] >= p.thresh;
+            if ((cand >> l) & 1ull) is_src = GROW ? true : scale * st.Q[(size_t)b * 64 + l] >= p.thresh;
             if (is_src) {
                 int32_t c[NDIM];
                 cell_coords<NDIM>(B, l, c);
@@ -193,7 +216,7 @@ __device__ void phase_targets(const Params& p, const Store& st, DevState* ds) {
             src |= (uint64_t)__ballot_sync(0xffffffffu, is_src) << (32 * hh);
         }
         if (!src) continue;
-        if (lane < ND) sAdj[w][lane] = st.adj[(size_t)b * ND + lane];
+        if (lane < ND) sAdj[w][lane] = my_adj;
         if (lane == 0) sQn[w] = 0u;
 #pragma unroll
         for (int d = 0; d < ND; ++d) {
@@ -201,7 +224,6 @@ __device__ void phase_targets(const Params& p, const Store& st, DevState* ds) {
                                           ((unsigned long long)__ballot_sync(0xffffffffu, (fl[1] >> d) & 1u) << 32);
             if (lane == 0) sO[w][d] = od;
         }
-        if (GROW && lane == 0) st.grown[b] = g | src;            // autonomous f: grow once
         __syncwarp();
         // ---- target classes: shift the source masks to the target slots, split by destination brick.
         // No atomics here: the parts bound for the own brick and the 2n face neighbours are merged
@@ -293,15 +315,16 @@ __device__ void phase_targets(const Params& p, const Store& st, DevState* ds) {
                 if (!GROW && row == NBR_NONE) row = ht_find(st.table, slots, key);
             }
             if (GROW) {
-                account(key, grow_apply(p, st, ds, NB0, slots, ND, row, key, bits));
+                grow_apply(p, st, ds, NB0, slots, ND, row, key, bits);
+                account(key, bits);
             } else if (row != NBR_NONE) {
                 const unsigned long long x = bits & st.mask[row];
                 if (x) atomicOr((unsigned long long*)&st.keep[row], x);
             }
         }
         __syncwarp();
-        if (GROW) {   // count the new cells and fold their CFL terms into the running maximum (Eq. 8):
-            // the queued (brick, bits) pairs are flattened so that every lane takes one new cell at a time
+        if (GROW) {   // fold the CFL terms of the target cells into the running maximum (Eq. 8):
+            // the queued (brick, bits) pairs are flattened so that every lane takes one cell at a time
             const unsigned nq = sQn[w];
             if (nq) {
                 unsigned run = 0;
@@ -328,22 +351,17 @@ __device__ void phase_targets(const Params& p, const Store& st, DevState* ds) {
                     int32_t TB[NDIM], tc[NDIM];
                     unpack<NDIM>(p, sQk[w][k], TB);
                     cell_coords<NDIM>(TB, tl, tc);
-                    double ul[NDIM], uu[NDIM];
-                    face_velocities<NDIM, DYN>(p, tc, ul, uu);
+                    double ul[NDIM];
+                    lower_face_velocities<NDIM, DYN>(p, tc, ul);
                     cfl_fold<NDIM>(p, ul, smax);
-                    ++n_new;
                 }
                 __syncwarp();
             }
         }
     }
     if (GROW) {
-        const double nn = block_sum((double)n_new);     // exact: counts << 2^53
         smax = block_max(smax);
-        if (threadIdx.x == 0) {
-            if (nn > 0.0) atomicAdd(&ds->N, (unsigned long long)nn);
-            if (smax > smax0) atomicMax(&ds->smax_bits, (unsigned long long)__double_as_longlong(smax));
-        }
+        if (threadIdx.x == 0 && smax > smax0) atomicMax(&ds->smax_bits, (unsigned long long)__double_as_longlong(smax));
     }
 }
 
@@ -391,8 +409,8 @@ __device__ void phase_smax(const Params& p, const Store& st, DevState* ds) {
         int32_t B[NDIM], c[NDIM];
         unpack<NDIM>(p, st.bkey[b], B);
         cell_coords<NDIM>(B, l, c);
-        double ul[NDIM], uu[NDIM];
-        face_velocities<NDIM, DYN>(p, c, ul, uu);
+        double ul[NDIM];
+        lower_face_velocities<NDIM, DYN>(p, c, ul);
         cfl_fold<NDIM>(p, ul, smax);
     }
     smax = block_max(smax);
@@ -400,33 +418,91 @@ __device__ void phase_smax(const Params& p, const Store& st, DevState* ds) {
 }
 
 // ---- a2+a4 pass 1: every active cell computes the fluxes of the faces it is UPWIND of -----------
-// Gather form D2 (= Eq. 7 + Alg. 1 + high-resolution term):
-//   T_l   = u+_{c,l}(P_c - P_{c-e^l}) + u-_{c+e^l,l}(P_{c+e^l} - P_c)
-//   G_j   = P*_{c,(j)} = P_c - sum_{l != j} 1/2 tau_l T_l
+// Gather form D2 (= Eq. 7 + Alg. 1 + high-resolution term), written in
+// Courant numbers a = tau_j u (tau_j = dt / h_j), so that every quantity below is tau_j * flux:
+//   T_l   = 1/2 [ a+_{c,l} (P_c - P_{c-e^l}) + a-_{c+e^l,l} (P_{c+e^l} - P_c) ]
+//   G_j   = P*_{c,(j)} = P_c - sum_{l != j} T_l
 //   sig_j = mc(P_c - P_{c-e^j}, P_{c+e^j} - P_c)     (limited wave when c is the upwind cell)
-//   upper face, u = u_{c+e^j,j} > 0:  F = u (G_j + 1/2 (1 - tau_j u) sig_j)
-//   lower face, u = u_{c,j}     < 0:  F = u (G_j - 1/2 (1 + tau_j u) sig_j)
-// A face whose upwind cell is NOT active carries only the high-resolution term; the active
-// downwind cell computes it (needs the two-hop value).
-// tau_j F goes to the downwind cell: through shared memory inside the brick, through phi[] across a
-// brick face (the downwind cell sets its fetch bit and picks it up in pass 2).
-// Qn <- P_c - sum_j tau_j (F_up - F_lo) over the faces resolved inside the brick.
-// Shared memory of one warp in pass 1: the brick's own row and its 2n neighbour rows (values and
-// activity flags), the update accumulator, the per-cell fetch flags and the list of active slots.
+//   upper face, a = a_{c+e^j,j} > 0:  F = a (G_j + 1/2 (1 - a) sig_j)
+//   lower face, a = a_{c,j}     < 0:  F = a (G_j - 1/2 (1 + a) sig_j)
+// A face whose upwind cell is NOT active carries only the high-resolution term; the active downwind
+// cell computes it (needs the two-hop value) and keeps it to itself.
+// F goes to both cells of the face: inside the brick through the face array Fb (written by the one
+// upwind owner, applied to both sides after the cell loop), across a brick face the owner applies it to
+// itself and leaves it in phi[] (the downwind cell sets its fetch bit and picks it up in pass 2).
+// Qn <- P_c - sum_j (F_up - F_lo) over the faces resolved inside the brick.
+//
+// Face velocities. Every dynamics id is affine in x_j for fixed other coordinates:
+// f_j(x) = A_j(x_{!=j}) + B_j x_j, so a_lo = tau_j A_j + (tau_j B_j) x_lo and a_up likewise with x_up:
+// one evaluation of A_j serves both faces, and the two cells of a face compute the same bits for its
+// Courant number (same A_j, same table entry for the face coordinate), which is what keeps "who is
+// upwind" consistent between them. The coordinates come from a per-brick table (2^K_j centres and
+// 2^K_j + 1 faces per dimension, A12 arithmetic). These Courant numbers serve the fluxes only; grow,
+// prune and dt use the unfused A12 velocities of gbees_common.cuh.
+template <int NDIM>
+struct FluxGeo {
+    using G = Geo<NDIM>;
+    __host__ __device__ static constexpr int XC(int j) { int o = 0; for (int m = 0; m < j; ++m) o += 1 << G::K(m); return o; }
+    __host__ __device__ static constexpr int XF(int j) { return XC(j) + j; }
+    static constexpr int NC = XC(NDIM), NF = XC(NDIM) + NDIM;
+};
+
+// Shared memory of one warp in pass 1
 template <int NDIM>
 struct alignas(16) Flux1Smem {
     static constexpr int ROWS = 2 * NDIM + 1, OWN = 2 * NDIM;
     double R[ROWS][64];              // staged rows: 2n neighbour bricks, then the brick itself
-    double acc[64];
-    unsigned long long M[ROWS];      // active masks of the staged rows
+    double Fb[NDIM][64];             // F through the UPPER j-face of slot l, faces inside the brick only
+    double acc[64];                  // P_c minus / plus the fluxes the cell applied to itself
+    double xc[FluxGeo<NDIM>::NC];    // cell-centre coordinates per dimension and local index
+    double xf[FluxGeo<NDIM>::NF];    // face coordinates: entry i = lower face of local index i
+    unsigned long long A[2 * NDIM];  // bit l of A[d]: the neighbour of slot l in direction d is active
+    unsigned long long RZ[2 * NDIM]; // bit l of RZ[d]: slot l active, that neighbour NOT active, the cell behind it active
     uint16_t fl[64];
     uint8_t list[64];
 };
+
+// A_j and B_j of f_j = A_j + B_j x_j (operation order fixed by the explicit intrinsics)
+template <int NDIM, int DYN>
+__device__ __forceinline__ double dyn_A(const Params& p, const double x[NDIM], int j) {
+    if constexpr (DYN == 0) {
+        if (j == 0) return DMUL(p.par[0], x[1]);
+        if (j == 1) return DMUL(x[0], DSUB(p.par[2], x[2]));
+        return DMUL(x[0], x[1]);
+    } else if constexpr (DYN == 1) {
+        if (j == 0) return DMUL(p.par[0], x[1]);
+        if (j == 1) return -DMUL(x[0], x[2]);
+        return __fma_rn(x[0], x[1], -DMUL(p.par[1], p.par[2]));
+    } else if constexpr (DYN == 2) {
+        const int jp = (j + 1) % NDIM, jm1 = (j + NDIM - 1) % NDIM, jm2 = (j + NDIM - 2) % NDIM;
+        return __fma_rn(DSUB(x[jp], x[jm2]), x[jm1], p.par[0]);
+    } else if constexpr (DYN == 3) {
+        double s = 0.0;
+#pragma unroll
+        for (int m = 0; m < NDIM; ++m) if (m != j) s = __fma_rn(p.par[j * NDIM + m], x[m], s);
+        return s;
+    } else {
+        return p.par[j];
+    }
+}
+template <int NDIM, int DYN>
+__device__ __forceinline__ double dyn_B(const Params& p, int j) {
+    if constexpr (DYN == 0) return j == 0 ? -p.par[0] : (j == 1 ? -1.0 : -p.par[1]);
+    else if constexpr (DYN == 1) return j == 0 ? -p.par[0] : (j == 1 ? -1.0 : -p.par[1]);
+    else if constexpr (DYN == 2) return -1.0;
+    else if constexpr (DYN == 3) return p.par[j * NDIM + j];
+    else return 0.0;
+}
+
+// sign tests on the high word (a value below 2^-1022 in magnitude counts as zero: its flux is zero anyway)
+__device__ __forceinline__ bool dpos(double a) { return __double2hiint(a) > 0; }
+__device__ __forceinline__ bool dneg(double a) { return __double2hiint(a) < 0; }
 
 // FAST = true: production setting (hi_res on, MC limiter) compiled in; false: flags read at run time
 template <int NDIM, int DYN, bool FAST>
 __device__ void phase_flux1(const Params& p, const Store& st, DevState* ds) {
     using G = Geo<NDIM>;
+    using FG = FluxGeo<NDIM>;
     using SM = Flux1Smem<NDIM>;
     constexpr int ND = 2 * NDIM, OWN = SM::OWN;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -436,143 +512,205 @@ __device__ void phase_flux1(const Params& p, const Store& st, DevState* ds) {
     const double dt = step_dt(p, ds);
     const bool hires = FAST || p.hi_res != 0, nolim = !FAST && p.limiter != 0;
     const double* __restrict__ Q = st.Q;
-    double tau[NDIM];
+    double tau[NDIM], tauB[NDIM];
 #pragma unroll
-    for (int j = 0; j < NDIM; ++j) tau[j] = dt / p.h[j];
+    for (int j = 0; j < NDIM; ++j) { tau[j] = dt / p.h[j]; tauB[j] = __dmul_rn(tau[j], (dyn_B<NDIM, DYN>(p, j))); }
+    // lane d < 2n builds the neighbour-activity masks of direction d: its geometry, once.
+    //   edge / w : slots whose step in direction d leaves the brick, and the shift that wraps them into the neighbour
+    //   edge2 / w2: the same for a step of two cells
+    unsigned long long my_edge = 0ull, my_edge2 = 0ull;
+    int my_s = 0, my_w = 0, my_w2 = 0;
+    if (lane < ND) {
+        const int j = lane >> 1, side = lane & 1;
+        my_edge = edge_mask<NDIM>(j, side);
+#pragma unroll
+        for (int m = 0; m < NDIM; ++m)
+            if (m == j) {
+                my_s = 1 << G::SH(m); my_w = G::MK(m) << G::SH(m); my_w2 = (G::MK(m) - 1) << G::SH(m);
+                for (int l = 0; l < 64; ++l) {
+                    const int lj = (l >> G::SH(m)) & G::MK(m);
+                    if (side ? lj + 2 > G::MK(m) : lj < 2) my_edge2 |= 1ull << l;
+                }
+            }
+    }
+    // coordinate-table entry t of this lane: dimension tj, local index ti (entries beyond the table: tj = -1)
+    constexpr uint32_t zrow = NBR_NONE;                     // missing neighbour brick: its staged row is zero-filled
+    const char* qlane = reinterpret_cast<const char*>(Q) + 16 * lane;
+    // metadata of the warp's next brick, loaded one brick ahead
+    uint32_t nx_row = zrow;
+    uint64_t nx_mask = 0ull, nx_bk = 0ull;
+    auto fetch_rows = [&](uint32_t bb) {
+        nx_row = zrow;
+        if (bb < NB) {
+            if (lane < ND) { const uint32_t a = st.adj[(size_t)bb * ND + lane]; if (a != NBR_NONE) nx_row = a; }
+            if (lane == OWN) nx_row = bb;
+            nx_bk = st.bkey[bb];
+        }
+    };
+    auto fetch_masks = [&]() { nx_mask = (lane <= OWN && nx_row != zrow) ? st.mask[nx_row] : 0ull; };
+    fetch_rows(gwarp());
+    fetch_masks();
+    unsigned ncells = 0;                                    // active cells of this warp's bricks (the grow does not count)
     for (uint32_t b = gwarp(); b < NB; b += gwarps()) {   // warp-uniform
         // ---- stage the 2n+1 rows (LDGSTS: 16 bytes per lane = one 512-byte row per warp instruction,
-        // no register round trip); rows of missing neighbour bricks are zero-filled; masks go to sm.M.
-        // (One 512-byte TMA bulk copy per row was measured too: equal on cfg2, 1.6x slower on cfg3s.)
-        uint32_t my_row = NBR_NONE;
-        uint64_t my_mask = 0ull;
-        if (lane < ND) my_row = st.adj[(size_t)b * ND + lane];
-        if (lane == OWN) my_row = b;
-        if (my_row != NBR_NONE) my_mask = st.mask[my_row];
-        const uint64_t bk = st.bkey[b];
-        if (lane < SM::ROWS) sm.M[lane] = my_mask;
+        // no register round trip); a missing neighbour brick is zero-filled by the same instruction.
+        const uint32_t my_row = nx_row;
+        const uint64_t my_mask = nx_mask, bk = nx_bk;
 #pragma unroll
         for (int r = 0; r < SM::ROWS; ++r) {
             const uint32_t row = __shfl_sync(0xffffffffu, my_row, r);
-            if (row != NBR_NONE) __pipeline_memcpy_async(&sm.R[r][2 * lane], &Q[(size_t)row * 64 + 2 * lane], 16);
-            else *reinterpret_cast<double2*>(&sm.R[r][2 * lane]) = make_double2(0.0, 0.0);
+            // (a missing brick copies nothing and zero-fills: the source address is only a placeholder)
+            __pipeline_memcpy_async(&sm.R[r][2 * lane], qlane + (size_t)(row == NBR_NONE ? b : row) * 512, 16, row == NBR_NONE ? 16 : 0);
         }
         __pipeline_commit();
+        fetch_rows(b + gwarps());                           // next brick: rows now, masks after the cell loop
+        // ---- while the rows are in flight: activity masks, coordinate tables, face array, cell list
         const uint64_t m = ((uint64_t)__shfl_sync(0xffffffffu, (uint32_t)(my_mask >> 32), OWN) << 32) |
                            __shfl_sync(0xffffffffu, (uint32_t)my_mask, OWN);
-        sm.acc[lane] = 0.0; sm.acc[lane + 32] = 0.0;
-        sm.fl[lane] = 0; sm.fl[lane + 32] = 0;
+        if (lane < ND) {
+            const bool up = lane & 1;
+            const unsigned long long a1 = ((up ? m >> my_s : m << my_s) & ~my_edge) |
+                                          ((up ? my_mask << my_w : my_mask >> my_w) & my_edge);
+            const unsigned long long a2 = ((up ? m >> 2 * my_s : m << 2 * my_s) & ~my_edge2) |
+                                          ((up ? my_mask << my_w2 : my_mask >> my_w2) & my_edge2);
+            sm.A[lane] = a1;
+            sm.RZ[lane] = nolim ? m & ~a1 : m & ~a1 & a2;      // without a limiter the wave needs no second cell
+        }
+        for (int t = (int)lane; t < FG::NF; t += 32) {
+            int tj = 0, ti = t;
+#pragma unroll
+            for (int j = 1; j < NDIM; ++j) if (t >= FG::XF(j)) { tj = j; ti = t - FG::XF(j); }
+            const int sh = (NDIM - 1 - tj) * p.bits;
+            const int32_t Bj = (int32_t)((int64_t)((bk >> sh) & ((1ull << p.bits) - 1ull)) - p.bias);
+            int kk = 0;
+#pragma unroll
+            for (int j = 0; j < NDIM; ++j) if (tj == j) kk = G::K(j);
+            const double ci = (double)(Bj * (1 << kk) + ti);
+            const double hj = p.h[tj], mj = p.mu[tj];
+            sm.xf[t] = DADD(mj, DMUL(ci - 0.5, hj));
+            if (ti < (1 << kk)) sm.xc[t - tj] = DADD(mj, DMUL(ci, hj));
+        }
+#pragma unroll
+        for (int j = 0; j < NDIM; ++j) *reinterpret_cast<double2*>(&sm.Fb[j][2 * lane]) = make_double2(0.0, 0.0);
         const uint32_t m_lo = (uint32_t)m, m_hi = (uint32_t)(m >> 32);
         const uint32_t below = (1u << lane) - 1u;
         if ((m_lo >> lane) & 1u) sm.list[__popc(m_lo & below)] = (uint8_t)lane;
         if ((m_hi >> lane) & 1u) sm.list[__popc(m_lo) + __popc(m_hi & below)] = (uint8_t)(lane + 32);
         const int cnt = __popcll(m);
-        int32_t B[NDIM];
-        unpack<NDIM>(p, bk, B);
+        ncells += (unsigned)cnt;
         __pipeline_wait_prior(0);
         __syncwarp();
         const double* Rf = &sm.R[0][0];
-        const unsigned long long* Mf = &sm.M[0];
-        for (int r0 = 0; r0 < cnt; r0 += 32) {             // active cells, 32 at a time
-            const bool act = r0 + (int)lane < cnt;
-            const int l = act ? sm.list[r0 + lane] : 0;
-            double q0 = 0.0, part = 0.0, S = 0.0;
-            double ul[NDIM], uu[NDIM], dm[NDIM], dp[NDIM], T[NDIM];
-            unsigned am = 0, ap = 0;                        // bit j: direct neighbour active
-            unsigned fl = 0;                                // bit d: fetch the flux of external face d in pass 2
-            if (act) {
-                q0 = sm.R[OWN][l];
-                int32_t c[NDIM];
-                cell_coords<NDIM>(B, l, c);
-                face_velocities<NDIM, DYN>(p, c, ul, uu);
+        // ---- cell loop: active cells, 32 at a time
+        for (int r0 = 0; r0 < cnt; r0 += 32) {
+            if (r0 + (int)lane >= cnt) continue;
+            const int l = sm.list[r0 + lane];
+            const double q0 = sm.R[OWN][l];
+            const unsigned lbit = 1u << (l & 31);
+            const unsigned* Aw = reinterpret_cast<const unsigned*>(&sm.A[0]) + (l >> 5);    // this cell's half of every mask
+            const unsigned* Zw = reinterpret_cast<const unsigned*>(&sm.RZ[0]) + (l >> 5);
+            double x[NDIM], al[NDIM], au[NDIM], dm[NDIM], dp[NDIM], T[NDIM];
 #pragma unroll
-                for (int j = 0; j < NDIM; ++j) {
-                    const int s = 1 << G::SH(j), MK = G::MK(j);
-                    const int lj = (l >> G::SH(j)) & MK;
-                    const int im = lj > 0 ? OWN * 64 + l - s : (2 * j) * 64 + l + MK * s;
-                    const int ip = lj < MK ? OWN * 64 + l + s : (2 * j + 1) * 64 + l - MK * s;
-                    const double vm = Rf[im], vp = Rf[ip];
-                    am |= (unsigned)((Mf[im >> 6] >> (im & 63)) & 1ull) << j;
-                    ap |= (unsigned)((Mf[ip >> 6] >> (ip & 63)) & 1ull) << j;
-                    dm[j] = q0 - vm;
-                    dp[j] = vp - q0;
-                    double t = 0.0;
-                    if (ul[j] > 0.0) t = ul[j] * dm[j];
-                    if (uu[j] < 0.0) t = fma(uu[j], dp[j], t);
-                    T[j] = (0.5 * tau[j]) * t;
-                    S += T[j];
-                }
-            }
+            for (int j = 0; j < NDIM; ++j) x[j] = sm.xc[FG::XC(j) + ((l >> G::SH(j)) & G::MK(j))];
+            double S = 0.0;
 #pragma unroll
             for (int j = 0; j < NDIM; ++j) {
                 const int s = 1 << G::SH(j), MK = G::MK(j);
-                int du = -1, dl = -1;         // in-brick destinations of the owned upper / lower face flux
-                double Fu = 0.0, Fl = 0.0;
-                if (act) {
-                    const int lj = (l >> G::SH(j)) & MK;
-                    const double Gj = (q0 - S) + T[j];     // P*_{c,(j)}
-                    const double sig = (hires && !nolim) ? mc_limit_fast(dm[j], dp[j]) : 0.0;
-                    const double tj = tau[j];
-                    const bool a_p = (ap >> j) & 1u, a_m = (am >> j) & 1u;
-                    {   // upper face of c
-                        const double u = uu[j];
-                        if (u > 0.0) {
-                            const double a = tj * u;
-                            const double wv = hires ? (nolim ? dp[j] : sig) : 0.0;
-                            const double F = a * fma(0.5 * (1.0 - a), wv, Gj);
+                const int lj = (l >> G::SH(j)) & MK;
+                const double tA = __dmul_rn(tau[j], (dyn_A<NDIM, DYN>(p, x, j)));
+                al[j] = __fma_rn(tauB[j], sm.xf[FG::XF(j) + lj], tA);
+                au[j] = __fma_rn(tauB[j], sm.xf[FG::XF(j) + lj + 1], tA);
+                double vm, vp;
+                if (G::K(j) == 1) {                // two cells along j: both neighbours sit at slot l ^ s, in the own row or across the face
+                    const double* nb = Rf + (l ^ s);
+                    vm = nb[(lj ? OWN : 2 * j) * 64];
+                    vp = nb[(lj ? 2 * j + 1 : OWN) * 64];
+                } else {
+                    vm = Rf[lj > 0 ? OWN * 64 + l - s : (2 * j) * 64 + l + MK * s];
+                    vp = Rf[lj < MK ? OWN * 64 + l + s : (2 * j + 1) * 64 + l - MK * s];
+                }
+                dm[j] = q0 - vm;
+                dp[j] = vp - q0;
+                double t = 0.0;
+                if (dpos(al[j])) t = al[j] * dm[j];
+                if (dneg(au[j])) t = fma(au[j], dp[j], t);
+                T[j] = 0.5 * t;
+                S += T[j];
+            }
+            double part = q0;
+            unsigned fl = 0;                                // bit d: fetch the flux of external face d in pass 2
+            const double qS = q0 - S;
+#pragma unroll
+            for (int j = 0; j < NDIM; ++j) {
+                const int s = 1 << G::SH(j), MK = G::MK(j);
+                const int lj = (l >> G::SH(j)) & MK;
+                const double Gj = qS + T[j];               // P*_{c,(j)}
+                const double sig = (hires && !nolim) ? mc_limit_fast(dm[j], dp[j]) : 0.0;
+                {   // upper face of c
+                    const double a = au[j];
+                    if (dpos(a)) {
+                        const double wv = hires ? (nolim ? dp[j] : sig) : 0.0;
+                        const double F = a * fma(0.5 - 0.5 * a, wv, Gj);
+                        if (lj < MK) sm.Fb[j][l] = F;
+                        else {
                             part -= F;
-                            if (a_p) {
-                                if (lj < MK) { du = l + s; Fu = F; }
-                                else st.phi[((size_t)b * ND + 2 * j + 1) * 32 + G::fidx(j, l)] = F;
-                            }
-                        } else if (u < 0.0) {
-                            if (a_p) {
-                                if (lj == MK) fl |= 1u << (2 * j + 1);
-                            } else if (hires) {   // upwind cell c+e^j inactive: W = 0 - P_c, W_up = P_{c+2e^j} - 0
-                                const int i2 = lj + 2 <= MK ? OWN * 64 + l + 2 * s : (2 * j + 1) * 64 + l + (1 - MK) * s;
-                                const double wv = nolim ? -q0 : mc_limit(-q0, Rf[i2]);
-                                const double a = tj * u;
-                                part -= (-0.5 * a) * (1.0 + a) * wv;
-                            }
+                            if (Aw[2 * (2 * j + 1)] & lbit) st.phi[((size_t)b * ND + 2 * j + 1) * 32 + G::fidx(j, l)] = F;
                         }
-                    }
-                    {   // lower face of c
-                        const double u = ul[j];
-                        if (u < 0.0) {
-                            const double a = tj * u;
-                            const double wv = hires ? (nolim ? dm[j] : sig) : 0.0;
-                            const double F = a * fma(-0.5 * (1.0 + a), wv, Gj);
-                            part += F;
-                            if (a_m) {
-                                if (lj > 0) { dl = l - s; Fl = F; }
-                                else st.phi[((size_t)b * ND + 2 * j) * 32 + G::fidx(j, l)] = F;
-                            }
-                        } else if (u > 0.0) {
-                            if (a_m) {
-                                if (lj == 0) fl |= 1u << (2 * j);
-                            } else if (hires) {   // upwind cell c-e^j inactive: W = P_c - 0, W_up = 0 - P_{c-2e^j}
-                                const int i2 = lj - 2 >= 0 ? OWN * 64 + l - 2 * s : (2 * j) * 64 + l + (MK - 1) * s;
-                                const double wv = nolim ? q0 : mc_limit(q0, -Rf[i2]);
-                                const double a = tj * u;
-                                part += (0.5 * a) * (1.0 - a) * wv;
-                            }
+                    } else if (dneg(a)) {
+                        if (lj == MK && (Aw[2 * (2 * j + 1)] & lbit)) fl |= 1u << (2 * j + 1);
+                        // upwind cell c+e^j inactive: W = 0 - P_c, W_up = P_{c+2e^j} - 0 (zero unless c+2e^j is active)
+                        if (hires && (Zw[2 * (2 * j + 1)] & lbit)) {
+                            const int i2 = lj + 2 <= MK ? OWN * 64 + l + 2 * s : (2 * j + 1) * 64 + l + (1 - MK) * s;
+                            const double wv = nolim ? dp[j] : mc_limit_fast(dp[j], Rf[i2]);
+                            part -= a * ((-0.5 - 0.5 * a) * wv);
                         }
                     }
                 }
-                // deliver inside the brick: for a fixed (j, side) the destinations are distinct
-                if (du >= 0) sm.acc[du] += Fu;
-                __syncwarp();
-                if (dl >= 0) sm.acc[dl] -= Fl;
-                __syncwarp();
+                {   // lower face of c
+                    const double a = al[j];
+                    if (dneg(a)) {
+                        const double wv = hires ? (nolim ? dm[j] : sig) : 0.0;
+                        const double F = a * fma(-0.5 - 0.5 * a, wv, Gj);
+                        if (lj > 0) sm.Fb[j][l - s] = F;
+                        else {
+                            part += F;
+                            if (Aw[2 * (2 * j)] & lbit) st.phi[((size_t)b * ND + 2 * j) * 32 + G::fidx(j, l)] = F;
+                        }
+                    } else if (dpos(a)) {
+                        if (lj == 0 && (Aw[2 * (2 * j)] & lbit)) fl |= 1u << (2 * j);
+                        // upwind cell c-e^j inactive: W = P_c - 0, W_up = 0 - P_{c-2e^j} (zero unless c-2e^j is active)
+                        if (hires && (Zw[2 * (2 * j)] & lbit)) {
+                            const int i2 = lj - 2 >= 0 ? OWN * 64 + l - 2 * s : (2 * j) * 64 + l + (MK - 1) * s;
+                            const double wv = nolim ? dm[j] : mc_limit_fast(dm[j], -Rf[i2]);
+                            part += a * ((0.5 - 0.5 * a) * wv);
+                        }
+                    }
+                }
             }
-            if (act) { sm.acc[l] += q0 + part; sm.fl[l] = (uint16_t)fl; }
-            __syncwarp();
+            sm.acc[l] = part;
+            sm.fl[l] = (uint16_t)fl;
         }
-        st.Qn[(size_t)b * 64 + lane] = sm.acc[lane];
-        st.Qn[(size_t)b * 64 + 32 + lane] = sm.acc[lane + 32];
-        st.fetch[(size_t)b * 64 + lane] = sm.fl[lane];
-        st.fetch[(size_t)b * 64 + 32 + lane] = sm.fl[lane + 32];
+        fetch_masks();                                      // next brick (its rows were fetched above)
+        __syncwarp();
+        // ---- apply the in-brick face fluxes to both of their cells, write the partial update
+#pragma unroll
+        for (int hh = 0; hh < 2; ++hh) {
+            const int l = (int)lane + 32 * hh;
+            const bool on = (m >> l) & 1ull;
+            double v = on ? sm.acc[l] : 0.0;
+#pragma unroll
+            for (int j = 0; j < NDIM; ++j) {
+                const int s = 1 << G::SH(j), MK = G::MK(j);
+                const int lj = (l >> G::SH(j)) & MK;
+                if (lj < MK) v -= sm.Fb[j][l];
+                if (lj > 0) v += sm.Fb[j][l - s];
+            }
+            st.Qn[(size_t)b * 64 + l] = on ? v : 0.0;
+            st.fetch[(size_t)b * 64 + l] = on ? sm.fl[l] : (uint16_t)0;
+        }
         __syncwarp();
     }
+    if (lane == 0 && ncells) atomicAdd(&ds->Ncount, (unsigned long long)ncells);
 }
 
 // ---- a5+a6 pass 2: fetch the fluxes owned by neighbour bricks, finish the update, sum the mass --
@@ -633,6 +771,7 @@ __device__ __forceinline__ void begin_step(DevState* ds) {
     ds->dt_cap = tt < 1e299 ? tt - t : 0.0;
     ds->N_before_grow = ds->N;
     ds->NB_before_grow = ds->NB;
+    ds->nsrc = 0u;
 }
 
 // one block: add the partials in index order, set the scale. after_step: advance t, count, flip
@@ -651,6 +790,9 @@ __device__ inline void finish_sum(const Params& p, const Store& st, DevState* ds
         if (p.normalise && v > 0.0) ds->scale = 1.0 / v;
         if (ds->N > p.max_cells) atomicOr(&ds->err, E_CAPACITY);
         if (after_step) {
+            ds->N = ds->Ncount;                    // pass 1 counted the grown grid
+            ds->Ncount = 0ull;
+            if (ds->N > p.max_cells) atomicOr(&ds->err, E_CAPACITY);
             const double dt = step_dt(p, ds);
             if (!(dt > 0.0)) atomicOr(&ds->err, E_DEGENERATE);
             ds->dt = dt;

@@ -38,6 +38,8 @@ struct Params {
 struct DevState {
     unsigned long long N;          // active cells
     unsigned long long N_before_grow;
+    unsigned long long Ncount;     // active cells counted by pass 1 of the running step
+    uint32_t nsrc;                 // bricks with new sources listed by this step's detect (slist / smask)
     uint32_t NB;                   // bricks in use (rows 0..NB-1)
     uint32_t NB_before_grow;       // bricks before this step's grow (link range start)
     int err;
@@ -78,6 +80,8 @@ struct Store {
     uint16_t* fetch;     // [capB][64] per cell: bit d = fetch the flux of external face d from the neighbour brick in pass 2
     uint32_t* adj;       // [capB][2n] neighbour brick rows: d = 2j (-e^j), 2j+1 (+e^j); NBR_NONE if absent
     uint32_t* slot_of;   // [capB] hashtable slot of a brick created by this step's grow
+    uint32_t* slist;     // [capB] rows of the bricks that hold new sources (this step's grow work list)
+    uint64_t* smask;     // [capB] their source masks
     ulonglong2* table;   // [slots] {brick key, row}
     uint64_t* pend;      // [slots] active bits set in bricks created during the running grow
     uint64_t* bkey2;     // compaction double buffers
@@ -228,6 +232,16 @@ __device__ __forceinline__ void face_velocities(const Params& p, const int32_t c
         ul[j] = dyn_f<NDIM, DYN>(p, x, j, xl);
         uu[j] = dyn_f<NDIM, DYN>(p, x, j, xu);
     }
+}
+
+// the n LOWER face velocities only (all Eq. 8 needs)
+template <int NDIM, int DYN>
+__device__ __forceinline__ void lower_face_velocities(const Params& p, const int32_t c[NDIM], double ul[NDIM]) {
+    double x[NDIM];
+#pragma unroll
+    for (int m = 0; m < NDIM; ++m) x[m] = DADD(p.mu[m], DMUL((double)c[m], p.h[m]));
+#pragma unroll
+    for (int j = 0; j < NDIM; ++j) ul[j] = dyn_f<NDIM, DYN>(p, x, j, DADD(p.mu[j], DMUL((double)c[j] - 0.5, p.h[j])));
 }
 
 // s_c = sum_j |u_{c,j}| / h_j, ascending j, true division (bit-identical to the oracle's Eq. 8 term)
