@@ -3,6 +3,7 @@
 // the launch-invariant inputs of init_gaussian / correct (an n x n Cholesky inverse, n <= 6).
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <utility>
@@ -21,7 +22,12 @@ using namespace gbees;
 #define GP const __grid_constant__ Params p, const __grid_constant__ Store st_in, DevState* ds
 #define ST const Store st = resolve(st_in, ds)
 // guard: 0 = always run, 1 = part of a step (runs if ds->go), 2 = part of a prune (runs if ds->prune_ok)
-#define GUARD(g) if (((g) == 1 && !ds->go) || ((g) == 2 && !ds->prune_ok)) return
+// Programmatic dependent launch: the kernels of a step / prune are enqueued with
+// cudaLaunchAttributeProgrammaticStreamSerialization, so the blocks of the next kernel may be scheduled
+// while the previous one drains. Every kernel first lets ITS dependents go, then waits until the kernel
+// before it has completed and flushed its memory -- before it reads anything, the go flag included.
+#define PDL_SYNC() do { asm volatile("griddepcontrol.launch_dependents;"); asm volatile("griddepcontrol.wait;" ::: "memory"); } while (0)
+#define GUARD(g) PDL_SYNC(); if (((g) == 1 && !ds->go) || ((g) == 2 && !ds->prune_ok)) return
 
 // start of gbees_step: one step with the caller's cap
 __global__ void k_begin_step(DevState* ds, double dt_cap) {
@@ -46,10 +52,11 @@ __global__ void __launch_bounds__(TPB) k_mark(GP) { GUARD(2); ST; phase_targets<
 template <int NDIM, bool ALL>
 __global__ void __launch_bounds__(TPB) k_link(GP, int guard) { GUARD(guard); ST; phase_link<NDIM, ALL>(p, st, ds); }
 template <int NDIM, int DYN, bool FAST>
-__global__ void __launch_bounds__(TPB) k_flux1(GP) { GUARD(1); ST; phase_flux1<NDIM, DYN, FAST>(p, st, ds); }
+__global__ void __launch_bounds__(TPB, 2) k_flux1(GP) { GUARD(1); ST; phase_flux1<NDIM, DYN, FAST>(p, st, ds); }
 // pass 2 + finish; a step that does not execute also cancels the prune enqueued behind it
 template <int NDIM>
-__global__ void __launch_bounds__(TPB) k_flux2(GP) {
+__global__ void __launch_bounds__(TPB, 8) k_flux2(GP) {
+    PDL_SYNC();
     if (!ds->go) { if (gtid() == 0) ds->prune_ok = 0; return; }
     ST;
     phase_flux2_finish<NDIM>(p, st, ds);
@@ -261,6 +268,7 @@ struct gbees_ctx {
     int no_grow = 0;
     int run_mode = 0;            // 0 = device-side step control, 1 = host loop over step/prune
     int small_ok = 1;            // the single-cluster persistent loop can be launched on this device
+    int pdl = 1;                 // programmatic dependent launch between the kernels of a step / prune
     int run_blocks_per_sm = 0;
     int64_t n_inserted = 0, n_pruned = 0;
     std::string err;
@@ -316,6 +324,18 @@ void drain_events(gbees_ctx* c) {   // call after a stream sync
 }
 
 template <int V> struct IC { static constexpr int value = V; };
+
+// enqueue one kernel of a step / prune (programmatic dependent launch unless switched off with GBEES_NO_PDL=1)
+template <typename... KArgs, typename... Args>
+void kl(gbees_ctx* c, void (*kern)(KArgs...), unsigned grid, unsigned block, size_t smem, Args&&... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = c->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = c->pdl;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, kern, KArgs(std::forward<Args>(args))...);
+}
 
 // call f(IC<NDIM>, IC<DYN>) for the context's (n, dynamics) pair; only valid pairs are instantiated
 template <typename F>
@@ -481,6 +501,7 @@ int gbees_create(gbees_ctx** out, int n, const double* dx, double threshold, int
     c->stream = (cudaStream_t)o.stream;
     c->no_grow = o.no_grow;
     c->run_mode = o.run_mode;
+    if (const char* e = std::getenv("GBEES_NO_PDL")) c->pdl = !(e[0] == '1');
     Params& p = c->p;
     p.n = n; p.dyn = dynamics_id;
     p.bits = 63 / n > 31 ? 31 : 63 / n;
@@ -638,17 +659,17 @@ static int enqueue_step(gbees_ctx* c) {
         constexpr int NN = decltype(N_)::value, DD = decltype(D_)::value;
         if (!c->no_grow) {
             phase(c, GBEES_PH_GROW, 2, [&] {
-                k_detect<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
-                k_grow<NN, DD><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
+                kl(c, k_detect, c->grid, TPB, 0, c->p, c->st, c->d_st);
+                kl(c, k_grow<NN, DD>, c->grid, TPB, 0, c->p, c->st, c->d_st);
             });
-            phase(c, GBEES_PH_LINK, 1, [&] { k_link<NN, false><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 1); });
+            phase(c, GBEES_PH_LINK, 1, [&] { kl(c, k_link<NN, false>, c->grid, TPB, 0, c->p, c->st, c->d_st, 1); });
         }
         phase(c, GBEES_PH_PASSA, 1, [&] {
             constexpr size_t smem = sizeof(Flux1Smem<NN>) * WPB;   // opt-in above 48 KB: set per device in gbees_create
-            if (c->p.hi_res && !c->p.limiter) k_flux1<NN, DD, true><<<c->grid_flux1, TPB, smem, c->stream>>>(c->p, c->st, c->d_st);
-            else k_flux1<NN, DD, false><<<c->grid_flux1, TPB, smem, c->stream>>>(c->p, c->st, c->d_st);
+            if (c->p.hi_res && !c->p.limiter) kl(c, k_flux1<NN, DD, true>, c->grid_flux1, TPB, smem, c->p, c->st, c->d_st);
+            else kl(c, k_flux1<NN, DD, false>, c->grid_flux1, TPB, smem, c->p, c->st, c->d_st);
         });
-        phase(c, GBEES_PH_PASSB, 1, [&] { k_flux2<NN><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st); });
+        phase(c, GBEES_PH_PASSB, 1, [&] { kl(c, k_flux2<NN>, c->grid, TPB, 0, c->p, c->st, c->d_st); });
         return GBEES_OK;
     });
     if (rc) return fail(c, rc, "unsupported (n, dynamics) pair");
@@ -659,18 +680,18 @@ static int enqueue_step(gbees_ctx* c) {
 static int enqueue_prune(gbees_ctx* c) {
     int rc = dispatch(c, [&](auto N_, auto D_) {
         constexpr int NN = decltype(N_)::value, DD = decltype(D_)::value;
-        phase(c, GBEES_PH_MARK, 1, [&] { k_mark<NN, DD><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st); });
+        phase(c, GBEES_PH_MARK, 1, [&] { kl(c, k_mark<NN, DD>, c->grid, TPB, 0, c->p, c->st, c->d_st); });
         phase(c, GBEES_PH_COMPACT, 4, [&] {
-            k_prune_scan<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
-            k_prune_move<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
-            k_zero_tail<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
-            k_after_compact<<<1, 1, 0, c->stream>>>(c->p, c->d_st);
+            kl(c, k_prune_scan, c->grid, TPB, 0, c->p, c->st, c->d_st);
+            kl(c, k_prune_move, c->grid, TPB, 0, c->p, c->st, c->d_st);
+            kl(c, k_zero_tail, c->grid, TPB, 0, c->p, c->st, c->d_st);
+            kl(c, k_after_compact, 1, 1, 0, c->p, c->d_st);
         });
         phase(c, GBEES_PH_REBUILD, 2, [&] {
-            k_clear_table<<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, 2);
-            k_prune_tail<NN, DD><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st);
+            kl(c, k_clear_table, c->grid, TPB, 0, c->p, c->st, c->d_st, 2);
+            kl(c, k_prune_tail<NN, DD>, c->grid, TPB, 0, c->p, c->st, c->d_st);
         });
-        phase(c, GBEES_PH_RELINK, 1, [&] { k_link_finish<NN><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, c->grid); });
+        phase(c, GBEES_PH_RELINK, 1, [&] { kl(c, k_link_finish<NN>, c->grid, TPB, 0, c->p, c->st, c->d_st, c->grid); });
         return GBEES_OK;
     });
     if (rc) return fail(c, rc, "unsupported (n, dynamics) pair");

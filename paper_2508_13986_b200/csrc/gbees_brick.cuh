@@ -445,6 +445,11 @@ struct FluxGeo {
     __host__ __device__ static constexpr int XC(int j) { int o = 0; for (int m = 0; m < j; ++m) o += 1 << G::K(m); return o; }
     __host__ __device__ static constexpr int XF(int j) { return XC(j) + j; }
     static constexpr int NC = XC(NDIM), NF = XC(NDIM) + NDIM;
+    // face array: one entry per in-brick face and dimension, addressed by the slot of the face's LOWER cell.
+    // When every dimension is two cells wide those slots have bit j clear: 32 entries per dimension do.
+    __host__ __device__ static constexpr bool all_two() { for (int j = 0; j < NDIM; ++j) if (G::K(j) != 1) return false; return true; }
+    static constexpr int FB = all_two() ? 32 : 64;
+    __host__ __device__ static constexpr int fb(int j, int l) { return all_two() ? G::fidx(j, l) : l; }
 };
 
 // Shared memory of one warp in pass 1
@@ -452,7 +457,7 @@ template <int NDIM>
 struct alignas(16) Flux1Smem {
     static constexpr int ROWS = 2 * NDIM + 1, OWN = 2 * NDIM;
     double R[ROWS][64];              // staged rows: 2n neighbour bricks, then the brick itself
-    double Fb[NDIM][64];             // F through the UPPER j-face of slot l, faces inside the brick only
+    double Fb[NDIM][FluxGeo<NDIM>::FB];   // F through the UPPER j-face of slot l, faces inside the brick only
     double acc[64];                  // P_c minus / plus the fluxes the cell applied to itself
     double xc[FluxGeo<NDIM>::NC];    // cell-centre coordinates per dimension and local index
     double xf[FluxGeo<NDIM>::NF];    // face coordinates: entry i = lower face of local index i
@@ -591,7 +596,8 @@ __device__ void phase_flux1(const Params& p, const Store& st, DevState* ds) {
             if (ti < (1 << kk)) sm.xc[t - tj] = DADD(mj, DMUL(ci, hj));
         }
 #pragma unroll
-        for (int j = 0; j < NDIM; ++j) *reinterpret_cast<double2*>(&sm.Fb[j][2 * lane]) = make_double2(0.0, 0.0);
+        for (int j = 0; j < NDIM; ++j)
+            if (2 * (int)lane < FG::FB) *reinterpret_cast<double2*>(&sm.Fb[j][2 * lane]) = make_double2(0.0, 0.0);
         const uint32_t m_lo = (uint32_t)m, m_hi = (uint32_t)(m >> 32);
         const uint32_t below = (1u << lane) - 1u;
         if ((m_lo >> lane) & 1u) sm.list[__popc(m_lo & below)] = (uint8_t)lane;
@@ -651,7 +657,7 @@ __device__ void phase_flux1(const Params& p, const Store& st, DevState* ds) {
                     if (dpos(a)) {
                         const double wv = hires ? (nolim ? dp[j] : sig) : 0.0;
                         const double F = a * fma(0.5 - 0.5 * a, wv, Gj);
-                        if (lj < MK) sm.Fb[j][l] = F;
+                        if (lj < MK) sm.Fb[j][FG::fb(j, l)] = F;
                         else {
                             part -= F;
                             if (Aw[2 * (2 * j + 1)] & lbit) st.phi[((size_t)b * ND + 2 * j + 1) * 32 + G::fidx(j, l)] = F;
@@ -671,7 +677,7 @@ __device__ void phase_flux1(const Params& p, const Store& st, DevState* ds) {
                     if (dneg(a)) {
                         const double wv = hires ? (nolim ? dm[j] : sig) : 0.0;
                         const double F = a * fma(-0.5 - 0.5 * a, wv, Gj);
-                        if (lj > 0) sm.Fb[j][l - s] = F;
+                        if (lj > 0) sm.Fb[j][FG::fb(j, l - s)] = F;
                         else {
                             part += F;
                             if (Aw[2 * (2 * j)] & lbit) st.phi[((size_t)b * ND + 2 * j) * 32 + G::fidx(j, l)] = F;
@@ -702,8 +708,8 @@ __device__ void phase_flux1(const Params& p, const Store& st, DevState* ds) {
             for (int j = 0; j < NDIM; ++j) {
                 const int s = 1 << G::SH(j), MK = G::MK(j);
                 const int lj = (l >> G::SH(j)) & MK;
-                if (lj < MK) v -= sm.Fb[j][l];
-                if (lj > 0) v += sm.Fb[j][l - s];
+                if (lj < MK) v -= sm.Fb[j][FG::fb(j, l)];
+                if (lj > 0) v += sm.Fb[j][FG::fb(j, l - s)];
             }
             st.Qn[(size_t)b * 64 + l] = on ? v : 0.0;
             st.fetch[(size_t)b * 64 + l] = on ? sm.fl[l] : (uint16_t)0;
@@ -726,9 +732,7 @@ __device__ void phase_flux2(const Params& p, const Store& st, DevState* ds) {
         if (lane < ND) my_nb = st.adj[(size_t)b * ND + lane];
         double a0 = st.Qn[(size_t)b * 64 + lane], a1 = st.Qn[(size_t)b * 64 + 32 + lane];
         const unsigned f0 = st.fetch[(size_t)b * 64 + lane], f1 = st.fetch[(size_t)b * 64 + 32 + lane];
-        unsigned any = f0 | f1;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) any |= __shfl_xor_sync(0xffffffffu, any, o);
+        const unsigned any = __reduce_or_sync(0xffffffffu, f0 | f1);
         if (any) {
 #pragma unroll
             for (int d = 0; d < ND; ++d) {
@@ -781,29 +785,47 @@ __device__ inline void finish_sum(const Params& p, const Store& st, DevState* ds
     for (unsigned k = threadIdx.x; k < nparts; k += blockDim.x) v += st.partial[k];
     v = block_sum(v);
     if (threadIdx.x == 0) {
+        // one thread closes the step: every field it needs is read up front (one round trip to L2 instead
+        // of a chain of them), the updates are plain stores
+        const double old = ds->scale, t0 = ds->t, tt = ds->t_target, cap = ds->dt_cap;
+        const unsigned long long N0 = ds->N, Nc = ds->Ncount, Nbg = ds->N_before_grow, steps = ds->steps,
+                                 limit = ds->step_limit, upd = ds->cell_updates, ins = ds->inserted_total,
+                                 sbits = ds->smax_bits;
+        const unsigned parity = ds->parity;
+        const uint32_t NBc = ds->NB;
+        int err = ds->err;
         ds->sumQ = v;
         if (!(v > 0.0) || !isfinite(v)) {
-            if (p.normalise || !isfinite(v)) atomicOr(&ds->err, E_DEGENERATE);
+            if (p.normalise || !isfinite(v)) err |= E_DEGENERATE;
         }
-        const double old = ds->scale;
         ds->mass = v * old;
         if (p.normalise && v > 0.0) ds->scale = 1.0 / v;
-        if (ds->N > p.max_cells) atomicOr(&ds->err, E_CAPACITY);
+        const unsigned long long N = after_step ? Nc : N0;      // pass 1 counted the grown grid
+        if (N > p.max_cells) err |= E_CAPACITY;
         if (after_step) {
-            ds->N = ds->Ncount;                    // pass 1 counted the grown grid
+            const double smax = __longlong_as_double((long long)sbits);
+            const bool capped = isfinite(cap) && cap > 0.0;      // same arithmetic as step_dt()
+            double dt = smax > 0.0 ? __ddiv_rn(p.cfl, smax) : (capped ? cap : 0.0);
+            if (capped && cap < dt) dt = cap;
+            if (!(dt > 0.0)) err |= E_DEGENERATE;
+            const double t1 = t0 + dt;
+            ds->N = N;
             ds->Ncount = 0ull;
-            if (ds->N > p.max_cells) atomicOr(&ds->err, E_CAPACITY);
-            const double dt = step_dt(p, ds);
-            if (!(dt > 0.0)) atomicOr(&ds->err, E_DEGENERATE);
             ds->dt = dt;
-            ds->t += dt;
-            ds->steps += 1;
-            ds->cell_updates += ds->N;
-            ds->inserted_total += ds->N - ds->N_before_grow;
-            ds->parity ^= 1u;
+            ds->t = t1;
+            ds->steps = steps + 1;
+            ds->cell_updates = upd + N;
+            ds->inserted_total = ins + (N - Nbg);
+            ds->parity = parity ^ 1u;
             ds->prune_ok = 1;
-            begin_step(ds);
+            // begin_step() for the next step, from the values at hand
+            ds->go = (t1 < tt) && (steps + 1 < limit) && err == 0 && N > 0ull;
+            ds->dt_cap = tt < 1e299 ? tt - t1 : 0.0;
+            ds->N_before_grow = N;
+            ds->NB_before_grow = NBc;
+            ds->nsrc = 0u;
         }
+        if (err) atomicOr(&ds->err, err);
     }
 }
 
