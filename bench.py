@@ -159,7 +159,7 @@ def run_reference(args, cfg):
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}))
 
 
-def run_cfg4(args):
+def cfg4_rows(key_counts, alphas):
     """BASELINE config 4: hashtable / compaction microbench (probes/op against PAPER.md:192, M ops/s,
     modelled GB/s: 16 B slot + 8 B key per insert / successful probe chain, 8 + 1 + 8 B per compacted key)."""
     import torch
@@ -172,14 +172,14 @@ def run_cfg4(args):
         torch.cuda.synchronize(); e0.record(); r = fn(); e1.record(); e1.synchronize()
         return r, e0.elapsed_time(e1) * 1e-3
 
-    for K in [int(k) for k in args.cfg4_keys.split(",")]:
+    for K in key_counts:
         keys = W.config4_keys(K)
         rng = np.random.default_rng(W.S0 + 42)
         dele = torch.from_numpy((rng.random(K) < 0.3).astype(np.uint8)).cuda()
         unit = np.uint64(1) << (np.uint64(10) * np.arange(6, dtype=np.uint64))
         sub = keys[:max(K // 12, 1)]
         q = torch.from_numpy(np.concatenate([sub + u for u in unit] + [sub - u for u in unit]).view(np.int64)).cuda()
-        for alpha in (0.3, 0.4, 0.5, 0.6, 0.7, 0.8):
+        for alpha in alphas:
             kt = torch.from_numpy(keys.view(np.int64)).cuda()
             ht = HashTable(int(np.ceil(K / alpha)))
             idx = torch.empty(K, dtype=torch.int32, device="cuda")
@@ -202,9 +202,98 @@ def run_cfg4(args):
                                                "GBps": q.numel() * (8 + 16 * p_nb / q.numel() + 4) / t_nb / 1e9},
                          "cooperative_probing": coop,
                          "delete30_compact_rebuild": {"survivors": kept, "Mkeys_per_s": K / t_cmp / 1e6}})
+    return rows
+
+
+def run_cfg4(args):
+    rows = cfg4_rows([int(k) for k in args.cfg4_keys.split(",")], (0.3, 0.4, 0.5, 0.6, 0.7, 0.8))
     print(json.dumps({"metric": "hashtable / compaction microbench (BASELINE config 4)", "unit": "probes/op, M ops/s, GB/s",
                       "n_gpus": 1, "data": "synthetic", "config": {"workload": "cfg4_hashtable", "keys": args.cfg4_keys},
                       "expected_probes": "PAPER.md:192: hit (1+1/(1-a))/2, miss (1+1/(1-a)^2)/2", "rows": rows}))
+
+
+KERNEL_OF_PHASE = {"grow": "k_detect + k_grow<{n},{d}>", "link": "k_link<{n},false>", "passA": "k_flux1<{n},{d},true>",
+                   "passB": "k_flux2<{n}>", "mark": "k_mark<{n},{d}>", "compact": "k_prune_scan + k_prune_move + k_zero_tail",
+                   "rebuild": "k_clear_table + k_prune_tail<{n},{d}>", "relink": "k_link_finish<{n}>", "correct": "k_correct<{n}>",
+                   "run": "k_run_small<{n},{d},true>"}
+
+
+def load_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        return json.load(open(path))["hbm_gbs"], "measured"
+    return 6650.0, "fallback"
+
+
+def measure(cfg, steps, warmup, local, stream, run_mode, flush, alpha=0.5, with_phases=True):
+    """Time `steps` jobs of one workload on the device (CUDA events on the launching stream, L2 flushed
+    between jobs); optionally one more job with per-phase event timing. Returns the context too."""
+    import torch
+    from paper_2508_13986_b200 import Gbees
+    n = cfg["n"]
+    g = Gbees(n, cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfg["cfl"], max_cells=cfg["max_cells"],
+              load_factor=alpha, device=local, stream=stream.cuda_stream, run_mode=run_mode)
+
+    def job(profile=False):
+        g.init_gaussian(cfg["mean"], cfg["cov"])
+        flush.zero_()
+        g.profile(profile)
+        l0 = g.stats()["launches"]
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        drive(g, cfg)
+        e1.record(stream)
+        e1.synchronize()
+        st = g.stats()
+        st["launches"] -= l0
+        return e0.elapsed_time(e1), st
+
+    for _ in range(warmup):
+        job()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    sampler.start()
+    ms_tot, upd_tot, launches, st = 0.0, 0, 0, None
+    for _ in range(steps):
+        ms, st = job()
+        ms_tot, upd_tot, launches = ms_tot + ms, upd_tot + st["cell_updates"], launches + st["launches"]
+    torch.cuda.synchronize()
+    clocks = sampler.result()
+    out = {"g": g, "job": job, "ms_tot": ms_tot, "upd_tot": upd_tot, "launches": launches, "stats": st, "clocks": clocks}
+    if with_phases:
+        _, st_prof = job(profile=True)
+        prof = g.profile(False)
+        pb = phase_bytes(st_prof, n, alpha)
+        out["phases"] = {k: {"ms": round(v[0], 4), "launches": v[1],
+                             "algo_GBps": (pb.get(k, 0) / (v[0] * 1e-3) / 1e9 if v[0] > 0 else None)}
+                         for k, v in prof.items() if v[1]}
+        out["phase_bytes"], out["st_prof"] = pb, st_prof
+    return out
+
+
+def extra_workloads(local, stream, run_mode, flush, peak, skip):
+    """The other BASELINE configs, 3 timed jobs each after 1 warm-up (north_star: throughput on the five
+    synthetic workloads). Short records: value, ms per job, whole-job roofline fraction, clocks."""
+    import torch
+    out = {}
+    for name in ("cfg0", "cfg1", "cfg3s", "cfg3"):
+        if name in skip:
+            continue
+        cfg = workload(name)
+        r = measure(cfg, 3, 1, local, stream, run_mode, flush, with_phases=False)
+        st, ms = r["stats"], r["ms_tot"] / 3
+        gbps = algo_bytes(st, cfg["n"], 0.5) / (ms * 1e-3) / 1e9
+        out[name] = {"workload": cfg["name"], "value": r["upd_tot"] / (r["ms_tot"] * 1e-3), "unit": UNIT, "ms_per_job": ms,
+                     "jobs": 3, "integration_steps_per_job": st["steps"], "prunes_per_job": st["prunes"],
+                     "cell_updates_per_job": st["cell_updates"], "final_cells": st["n_cells"],
+                     "whole_job_algo_GBps": gbps, "whole_job_frac": gbps / peak, "gpu_launches": r["launches"],
+                     "clocks": r["clocks"]}
+        r["g"].close()
+        del r
+        torch.cuda.empty_cache()
+    if "cfg4" not in skip:
+        out["cfg4"] = cfg4_rows([1000000, 10000000], (0.5,))
+    return out
 
 
 def main():
@@ -215,6 +304,7 @@ def main():
     ap.add_argument("--workload", default="cfg2")
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extra", action="store_true", help="skip the short records of the other workloads (\"workloads\" in the JSON line)")
     ap.add_argument("--cfg4-keys", default="1000000,10000000", help="key counts of the cfg4 microbench (1e8 needs ~25 GB)")
     ap.add_argument("--run-mode", type=int, default=0, help="gbees_run: 0 = device-side step control (no host round trip per step), 1 = host loop of gbees_step/gbees_prune")
     args = ap.parse_args()
@@ -226,7 +316,6 @@ def main():
 
     import torch
     import torch.distributed as dist
-    from paper_2508_13986_b200 import Gbees
     rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     assert torch.cuda.is_available(), "bench.py needs a CUDA device: there is no CPU fallback"
@@ -235,63 +324,32 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     n, alpha = cfg["n"], 0.5
     stream = torch.cuda.Stream()
+    peak, peak_src = load_peak()
     with torch.cuda.stream(stream):
-        g = Gbees(n, cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfg["cfl"], max_cells=cfg["max_cells"],
-                  load_factor=alpha, device=local, stream=stream.cuda_stream, run_mode=args.run_mode)
         flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2
-
-        def job(profile=False):
-            g.init_gaussian(cfg["mean"], cfg["cov"])
-            flush.zero_()
-            g.profile(profile)
-            l0 = g.stats()["launches"]
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record(stream)
-            drive(g, cfg)
-            e1.record(stream)
-            e1.synchronize()
-            st = g.stats()
-            st["launches"] -= l0
-            return e0.elapsed_time(e1), st
-
-        for _ in range(max(args.warmup, 3)):
-            job()
         if world > 1:
             dist.barrier()
-        torch.cuda.synchronize()
-        sampler = ClockSampler(local)
-        sampler.start()
-        ms_tot, upd_tot, launches, st = 0.0, 0, 0, None
-        for _ in range(args.steps):
-            ms, st = job()
-            ms_tot, upd_tot, launches = ms_tot + ms, upd_tot + st["cell_updates"], launches + st["launches"]
-        torch.cuda.synchronize()
-        clocks = sampler.result()
-        ms_max, upd_all = aggregate(ms_tot, upd_tot, "cuda")
-
-        # per-phase CUDA-event timing of one more job (same workload, same launch configuration)
-        ms_prof, st_prof = job(profile=True)
-        prof = g.profile(False)
-        pb = phase_bytes(st_prof, n, alpha)
-        phases = {k: {"ms": round(v[0], 4), "launches": v[1],
-                      "algo_GBps": (pb.get(k, 0) / (v[0] * 1e-3) / 1e9 if v[0] > 0 else None)}
-                  for k, v in prof.items() if v[1]}
+        r = measure(cfg, args.steps, max(args.warmup, 3), local, stream, args.run_mode, flush, alpha)
+        g, st, ms_tot, clocks, launches = r["g"], r["stats"], r["ms_tot"], r["clocks"], r["launches"]
+        ms_max, upd_all = aggregate(ms_tot, r["upd_tot"], "cuda")
+        phases, pb, st_prof = r["phases"], r["phase_bytes"], r["st_prof"]
         dom = max(phases, key=lambda k: phases[k]["ms"])
-        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))) if os.path.exists(
-            os.path.join(ROOT, "MEASURED_PEAKS.json")) else None
-        peak, peak_src = (peaks["hbm_gbs"], "measured") if peaks else (6650.0, "fallback")
         job_GBps = algo_bytes(st, n, alpha) / (ms_tot / args.steps * 1e-3) / 1e9
         dom_GBps = phases[dom]["algo_GBps"] or 0.0
-        # measured DRAM traffic of the dominant kernel, from the committed ncu --set full capture (bytes per cell-update)
-        traffic = None
+        # DRAM traffic of the dominant kernel: bytes per cell-update from the committed ncu --set full capture
+        # (profiles/traffic.json, a static figure) times the live cell count
+        traffic, traffic_src = None, None
         tpath = os.path.join(ROOT, "profiles", "traffic.json")
         if os.path.exists(tpath):
             tj = json.load(open(tpath))
             if tj.get("phase") == dom and tj.get("workload") == cfg["name"]:
                 traffic = tj["dram_bytes_per_cell_update"] * st_prof["cell_updates"] / max(phases[dom]["launches"], 1)
-        roofline = {"bound": "hbm", "kernel": dom, "achieved": dom_GBps, "peak": peak, "unit": "GB/s",
-                    "frac": dom_GBps / peak, "traffic": traffic, "peak_source": peak_src,
+                traffic_src = "profiles/traffic.json (static: ncu capture of an earlier run x live cell count)"
+        kname = KERNEL_OF_PHASE.get(dom, dom).format(n=n, d=cfg["dyn"])
+        roofline = {"bound": "hbm", "kernel": kname, "phase": dom, "achieved": dom_GBps, "peak": peak, "unit": "GB/s",
+                    "frac": dom_GBps / peak, "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
                     "algo_bytes_per_launch": pb.get(dom, 0) / max(phases[dom]["launches"], 1),
+                    "timing": "CUDA events around every launch of the phase in one extra job (event timing switches the programmatic dependent launch overlap off, so the phases add up to more than ms_per_step)",
                     "whole_job": {"achieved": job_GBps, "frac": job_GBps / peak,
                                   "frac_of_8TBps": job_GBps / 8000.0, "algo_bytes_per_job": algo_bytes(st, n, alpha)},
                     "phases": phases}
@@ -315,9 +373,14 @@ def main():
                 dt_ = time.perf_counter() - t0
                 if it >= 2:
                     e2e_ms += 1e3 * dt_; e2e_upd += g.stats()["cell_updates"]; d2h = cnt.value * (4 * n + 8)
+            del hk, hp
         e2e = {"value": (e2e_upd / (e2e_ms * 1e-3) * world) if e2e_ms else None, "unit": UNIT,
                "h2d_bytes_per_step": 8 * (n + n * n), "d2h_bytes_per_step": d2h,
                "ms_per_step": e2e_ms / args.steps if e2e_ms else None}
+        g.close()
+        workloads = None
+        if rank == 0 and world == 1 and not args.no_extra:
+            workloads = extra_workloads(local, stream, args.run_mode, flush, peak, skip={args.workload})
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -335,7 +398,8 @@ def main():
                        "cell_updates_per_job": st["cell_updates"], "final_cells": st["n_cells"],
                        "parallelism": "replicas only" if world > 1 else "1 GPU", "run_mode": args.run_mode,
                        "l2": "256 MiB memset between jobs (flush)"},
-            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu}))
+            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
+            "workloads": workloads}))
     if world > 1:
         dist.destroy_process_group()
 

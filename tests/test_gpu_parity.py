@@ -6,7 +6,7 @@ import pytest
 
 from oracle.binding import Oracle
 from paper_2508_13986_b200 import workloads as W
-from util import compare_states
+from util import compare_states, key_hash, sort_state
 
 pytestmark = pytest.mark.gpu
 
@@ -242,6 +242,82 @@ def test_config2_full_size_against_oracle_golden():
     assert g2.run(cfg["t_end"], prune_every=cfg["prune_every"]) == gold["steps"]
     k2, p2 = g2.export()
     assert np.array_equal(k2, gk) and np.max(np.abs(p2 - gp)) <= 1e-12 * gp.max()
+
+
+def test_config2_full_size_every_cell_against_the_live_oracle():
+    """BASELINE config 2 (the headline) at full size, element by element (north_star: identical active cell
+    sets, probabilities within 1e-10 per step / 1e-8 after the run; compare every 10th step +
+    final). The oracle runs live beside the GPU (about 4.5 minutes on one host core); the GPU goes through
+    gbees_run with device-side step control and prune_every = 5, the launch configuration bench.py times."""
+    cfg = W.config2()
+    o = Oracle(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfg["cfl"])
+    g = G(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfg["cfl"], max_cells=cfg["max_cells"])
+    o.init_gaussian(cfg["mean"], cfg["cov"]); g.init_gaussian(cfg["mean"], cfg["cov"])
+    k, worst = 0, 0.0
+    while o.time() < cfg["t_end"]:
+        k0 = k
+        while k < k0 + 10 and o.time() < cfg["t_end"]:
+            o.step(cfg["t_end"] - o.time()); k += 1
+            if k % cfg["prune_every"] == 0:
+                o.prune()
+        assert g.run(cfg["t_end"], max_steps=10, prune_every=cfg["prune_every"]) == k - k0
+        assert g.time() == o.time()                          # dt bit-identical step after step (A12)
+        gk, gp = sort_state(*g.export(sort=False)); ok, op = sort_state(*o.export(sort=False))
+        assert np.array_equal(gk, ok), f"step {k}: active sets differ ({len(gk)} vs {len(ok)} cells)"
+        err = np.max(np.abs(gp - op)) / np.max(np.abs(op))
+        worst = max(worst, err)
+        assert err <= 1e-10 * k, f"step {k}: max-norm relative error {err:.3e}"   # 1e-10 per step, compounded
+    assert k == 105 and len(gp) == 877679
+    assert worst <= 1e-8
+    assert gp.sum() == pytest.approx(1.0, abs=1e-12)
+
+
+def test_config3_tenth_scale_full_run_against_oracle_golden():
+    """The 1/10-scale twin of BASELINE config 3 (dx = 0.5, 6 M -> 10 M cells, all 50 steps, prune every 5;
+    SURVEY.md 8(d)) against the oracle's stored result (tests/golden/cfg3s_full_oracle.json, written by
+    tests/golden/make_cfg3s_golden.py, which calls only oracle/ and takes hours): after EVERY prune the cell
+    count and the sha256 of the sorted int32 key array (bit-exact active sets); at the end 4096 sampled
+    masses (1e-8), the six 1-D marginals and the first two moments. A golden file from an interrupted
+    generator run holds fewer prunes: whatever it holds is compared."""
+    import json
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "cfg3s_full_oracle.json")
+    if not os.path.exists(path):
+        pytest.skip("tests/golden/cfg3s_full_oracle.json has not been generated")
+    gold = json.load(open(path))
+    cfg = W.config3(dx=0.5)
+    g = G(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfg["cfl"], max_cells=1 << 25)
+    g.init_gaussian(cfg["mean"], cfg["cov"])
+    assert g.count() == gold["cells_initial"]
+    done = 0
+    for k in sorted(int(x) for x in gold["after_prune"]):
+        assert g.run(1e300, max_steps=k - done, prune_every=cfg["prune_every"]) == k - done
+        done = k
+        want = gold["after_prune"][str(k)]
+        assert g.count() == want["cells"], f"cell count after the prune at step {k}"
+        assert g.time() == pytest.approx(want["t"], rel=1e-13)
+        ks, ps = sort_state(*g.export(sort=False))
+        assert key_hash(ks) == want["keys_sha256"], f"active set after the prune at step {k}"
+        assert ps.max() == pytest.approx(want["p_max"], rel=1e-8)
+    assert done >= 5
+    if "final" in gold:
+        f = gold["final"]
+        assert done == f["steps"] == cfg["steps"] and len(ps) == f["cells"]
+        # sampled masses: the sample keys are looked up in the sorted GPU state through the packed sort key
+        sk = np.asarray(f["sample_keys"], dtype=np.int32)
+        pack = lambda a: sum((a[:, j].astype(np.int64) + 512) << (10 * (5 - j)) for j in range(6))
+        pos = np.searchsorted(pack(ks), pack(sk))
+        assert np.array_equal(ks[pos], sk)                   # every sampled key is active
+        assert np.max(np.abs(ps[pos] - np.asarray(f["sample_p"]))) <= 1e-8 * f["p_max"]
+        x = ks.astype(np.float64)
+        mean = ps @ x
+        d = x - mean
+        assert np.allclose(mean, f["mean_index_units"], rtol=0, atol=1e-8)
+        assert np.allclose(d.T @ (d * ps[:, None]), f["cov_index_units"], rtol=1e-8, atol=1e-8)
+        for j, mg in enumerate(f["marginals_1d"]):
+            u, inv = np.unique(ks[:, j], return_inverse=True)
+            assert u.tolist() == mg["coords"]
+            assert np.allclose(np.bincount(inv, weights=ps), mg["mass"], rtol=0, atol=1e-10)
 
 
 def test_config1_full_run_with_corrections_bench_sequence():

@@ -26,3 +26,22 @@ def compare_states(gk, gp, ok, op, thresh, rtol, band=1e-12, what=""):
     err = np.max(np.abs(gp[common_g] - op[common_o])) / np.max(np.abs(op))
     assert err <= rtol, f"{what}: max-norm relative error {err:.3e} > {rtol:.1e}"
     return err
+
+
+def sort_state(keys, p):
+    """Lexicographic order (dimension 0 most significant) through one packed int64 key per cell
+    (10 bits per coordinate for n = 6, i.e. |c| < 512: the packable range of the product itself)."""
+    keys = np.ascontiguousarray(keys, dtype=np.int32)
+    n = keys.shape[1]
+    bits = 63 // n if 63 // n < 31 else 31
+    code = np.zeros(len(keys), dtype=np.int64)
+    for j in range(n):
+        code = (code << bits) | (keys[:, j].astype(np.int64) + (1 << (bits - 1)))
+    order = np.argsort(code, kind="stable")
+    return np.ascontiguousarray(keys[order]), np.asarray(p)[order]
+
+
+def key_hash(keys_sorted):
+    """sha256 of the sorted int32 key array (bit-exact active-set fingerprint)."""
+    import hashlib
+    return hashlib.sha256(np.ascontiguousarray(keys_sorted, dtype=np.int32).tobytes()).hexdigest()
