@@ -51,8 +51,10 @@ template <int NDIM, int DYN>
 __global__ void __launch_bounds__(TPB) k_mark(GP) { GUARD(2); ST; phase_targets<NDIM, DYN, false>(p, st, ds); }
 template <int NDIM, bool ALL>
 __global__ void __launch_bounds__(TPB) k_link(GP, int guard) { GUARD(guard); ST; phase_link<NDIM, ALL>(p, st, ds); }
+// pass 1 runs FLUX1_WPB warps per block, 2 blocks per SM (register-capped: 65536 / (2 x 32 x FLUX1_WPB) per thread)
+constexpr int FLUX1_WPB = 8;
 template <int NDIM, int DYN, bool FAST>
-__global__ void __launch_bounds__(TPB, 2) k_flux1(GP) { GUARD(1); ST; phase_flux1<NDIM, DYN, FAST>(p, st, ds); }
+__global__ void __launch_bounds__(32 * FLUX1_WPB, 2) k_flux1(GP) { GUARD(1); ST; phase_flux1<NDIM, DYN, FAST>(p, st, ds); }
 // pass 2 + finish; a step that does not execute also cancels the prune enqueued behind it
 template <int NDIM>
 __global__ void __launch_bounds__(TPB, 8) k_flux2(GP) {
@@ -538,7 +540,7 @@ int gbees_create(gbees_ctx** out, int n, const double* dx, double threshold, int
     // dynamic shared memory above 48 KB is an opt-in per function AND per device: set it for this context's device
     if (dispatch(c, [&](auto N_, auto D_) {
             constexpr int NN = decltype(N_)::value, DD = decltype(D_)::value;
-            constexpr int smem = (int)(sizeof(Flux1Smem<NN>) * WPB);
+            constexpr int smem = (int)(sizeof(Flux1Smem<NN>) * FLUX1_WPB);
             if (cudaFuncSetAttribute(k_flux1<NN, DD, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess ||
                 cudaFuncSetAttribute(k_flux1<NN, DD, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
                 return GBEES_ERR_CUDA;
@@ -665,9 +667,9 @@ static int enqueue_step(gbees_ctx* c) {
             phase(c, GBEES_PH_LINK, 1, [&] { kl(c, k_link<NN, false>, c->grid, TPB, 0, c->p, c->st, c->d_st, 1); });
         }
         phase(c, GBEES_PH_PASSA, 1, [&] {
-            constexpr size_t smem = sizeof(Flux1Smem<NN>) * WPB;   // opt-in above 48 KB: set per device in gbees_create
-            if (c->p.hi_res && !c->p.limiter) kl(c, k_flux1<NN, DD, true>, c->grid_flux1, TPB, smem, c->p, c->st, c->d_st);
-            else kl(c, k_flux1<NN, DD, false>, c->grid_flux1, TPB, smem, c->p, c->st, c->d_st);
+            constexpr size_t smem = sizeof(Flux1Smem<NN>) * FLUX1_WPB;   // opt-in above 48 KB: set per device in gbees_create
+            if (c->p.hi_res && !c->p.limiter) kl(c, k_flux1<NN, DD, true>, c->grid_flux1, 32 * FLUX1_WPB, smem, c->p, c->st, c->d_st);
+            else kl(c, k_flux1<NN, DD, false>, c->grid_flux1, 32 * FLUX1_WPB, smem, c->p, c->st, c->d_st);
         });
         phase(c, GBEES_PH_PASSB, 1, [&] { kl(c, k_flux2<NN>, c->grid, TPB, 0, c->p, c->st, c->d_st); });
         return GBEES_OK;

@@ -445,11 +445,11 @@ struct FluxGeo {
     __host__ __device__ static constexpr int XC(int j) { int o = 0; for (int m = 0; m < j; ++m) o += 1 << G::K(m); return o; }
     __host__ __device__ static constexpr int XF(int j) { return XC(j) + j; }
     static constexpr int NC = XC(NDIM), NF = XC(NDIM) + NDIM;
-    // face array: one entry per in-brick face and dimension, addressed by the slot of the face's LOWER cell.
-    // When every dimension is two cells wide those slots have bit j clear: 32 entries per dimension do.
-    __host__ __device__ static constexpr bool all_two() { for (int j = 0; j < NDIM; ++j) if (G::K(j) != 1) return false; return true; }
-    static constexpr int FB = all_two() ? 32 : 64;
-    __host__ __device__ static constexpr int fb(int j, int l) { return all_two() ? G::fidx(j, l) : l; }
+    // face array: one entry per in-brick face and dimension, addressed by the slot of the face's LOWER cell
+    // (64 entries per dimension; packing them to the 32 that a two-cell-wide dimension uses costs more index
+    // arithmetic per cell than the shared memory is worth while registers cap the occupancy at 2 blocks per SM)
+    static constexpr int FB = 64;
+    __host__ __device__ static constexpr int fb(int, int l) { return l; }
 };
 
 // Shared memory of one warp in pass 1
@@ -540,15 +540,15 @@ __device__ void phase_flux1(const Params& p, const Store& st, DevState* ds) {
     }
     // coordinate-table entry t of this lane: dimension tj, local index ti (entries beyond the table: tj = -1)
     constexpr uint32_t zrow = NBR_NONE;                     // missing neighbour brick: its staged row is zero-filled
-    const char* qlane = reinterpret_cast<const char*>(Q) + 16 * lane;
+    const uint64_t qlane = reinterpret_cast<uint64_t>(Q) + 16ull * lane;
     // metadata of the warp's next brick, loaded one brick ahead
     uint32_t nx_row = zrow;
     uint64_t nx_mask = 0ull, nx_bk = 0ull;
-    auto fetch_rows = [&](uint32_t bb) {
+    auto fetch_rows = [&](uint32_t bb) {   // (nothing here may USE what it loads: the loads stay in flight behind the cell loop)
         nx_row = zrow;
         if (bb < NB) {
-            if (lane < ND) { const uint32_t a = st.adj[(size_t)bb * ND + lane]; if (a != NBR_NONE) nx_row = a; }
-            if (lane == OWN) nx_row = bb;
+            if (lane < ND) nx_row = st.adj[(size_t)bb * ND + lane];     // NBR_NONE = zrow: a missing neighbour
+            else if (lane == OWN) nx_row = bb;
             nx_bk = st.bkey[bb];
         }
     };
@@ -565,7 +565,7 @@ __device__ void phase_flux1(const Params& p, const Store& st, DevState* ds) {
         for (int r = 0; r < SM::ROWS; ++r) {
             const uint32_t row = __shfl_sync(0xffffffffu, my_row, r);
             // (a missing brick copies nothing and zero-fills: the source address is only a placeholder)
-            __pipeline_memcpy_async(&sm.R[r][2 * lane], qlane + (size_t)(row == NBR_NONE ? b : row) * 512, 16, row == NBR_NONE ? 16 : 0);
+            __pipeline_memcpy_async(&sm.R[r][2 * lane], reinterpret_cast<const void*>(qlane + (uint64_t)(row == NBR_NONE ? b : row) * 512ull), 16, row == NBR_NONE ? 16 : 0);
         }
         __pipeline_commit();
         fetch_rows(b + gwarps());                           // next brick: rows now, masks after the cell loop

@@ -631,3 +631,47 @@ def test_F3_marginal_oracle_pins():
     assert m02.sum() == pytest.approx(p.sum(), rel=1e-14)
     kall, mall = MO.marginal(keys, p, [0, 1, 2])
     assert np.array_equal(kall, keys) and np.array_equal(mall, p)
+
+
+def test_F1b_resample_oracle_pins():
+    """Conservative remap between grids of different spacing (reading A19; spatial convergence):
+    mass is preserved, the same grid gives the same PDF, a product measure remaps factor by factor, a 3:1
+    nested grid is the plain sum over the 3^n children, and a uniform density stays uniform."""
+    from oracle import resample_oracle as RO
+    rng = np.random.default_rng(S0 + 401)
+    # (1) mass, (2) identity
+    keys = box([-3, -2, -4], [4, 3, 2])
+    keys = keys[rng.random(len(keys)) < 0.7]
+    p = rng.random(len(keys)) - 0.1                                    # negatives are kept (A5)
+    o, h = np.array([0.3, -1.0, 2.0]), np.array([0.5, 0.25, 0.4])
+    o2, h2 = np.array([0.1, -0.9, 2.3]), np.array([0.8, 0.3, 0.4])
+    k2, p2 = RO.resample(keys, p, o, h, o2, h2)
+    assert p2.sum() == pytest.approx(p.sum(), rel=1e-13)
+    ks, ps = RO.resample(keys, p, o, h, o, h)
+    order = np.lexsort(keys.T[::-1])
+    assert np.array_equal(ks, keys[order]) and np.allclose(ps, p[order], rtol=1e-15, atol=0)
+    # (3) product measure: remap of a product = product of the 1-D remaps
+    a, b = rng.random(7), rng.random(5)
+    kk = np.array([[i, j] for i in range(7) for j in range(5)], dtype=np.int32) - 2
+    pp = np.array([a[i] * b[j] for i in range(7) for j in range(5)])
+    oo, hh, oo2, hh2 = np.array([0.0, 1.0]), np.array([0.5, 0.5]), np.array([0.2, 1.0]), np.array([0.8, 1.25])
+    k2d, p2d = RO.resample(kk, pp, oo, hh, oo2, hh2)
+    ka, pa = RO.resample(np.arange(7).reshape(-1, 1) - 2, a, oo[:1], hh[:1], oo2[:1], hh2[:1])
+    kb, pb = RO.resample(np.arange(5).reshape(-1, 1) - 2, b, oo[1:], hh[1:], oo2[1:], hh2[1:])
+    want = {(int(x), int(y)): u * v for x, u in zip(ka[:, 0], pa) for y, v in zip(kb[:, 0], pb)}
+    assert len(k2d) == len(want)
+    assert all(abs(want[tuple(k)] - v) <= 1e-14 for k, v in zip(k2d.tolist(), p2d.tolist()))
+    # (4) nested 3:1 grid with a common origin: coarse cell d = sum of the fine cells 3d-1, 3d, 3d+1 per dimension
+    kf = box([-4, -4], [5, 5])
+    pf = rng.random(len(kf))
+    kc, pc = RO.resample(kf, pf, np.zeros(2), np.array([0.2, 0.2]), np.zeros(2), np.array([0.6, 0.6]))
+    lut = {tuple(k): v for k, v in zip(kf.tolist(), pf.tolist())}
+    for d, v in zip(kc.tolist(), pc.tolist()):
+        s = sum(lut.get((3 * d[0] + i, 3 * d[1] + j), 0.0) for i in (-1, 0, 1) for j in (-1, 0, 1))
+        assert v == pytest.approx(s, rel=1e-13)
+    assert len(kc) == 9
+    # (5) 1-D uniform density rho on cells -10..10 (h = 0.3): interior cells of the h2 = 0.7 grid get rho * h2
+    k1 = np.arange(-10, 11).reshape(-1, 1).astype(np.int32)
+    kq, pq = RO.resample(k1, np.full(21, 2.0 * 0.3), np.array([0.05]), np.array([0.3]), np.array([0.0]), np.array([0.7]))
+    inner = np.abs(kq[:, 0]) <= 3
+    assert np.allclose(pq[inner], 2.0 * 0.7, rtol=1e-13)
