@@ -143,6 +143,17 @@ int gbees_compare(gbees_ctx* ctx, gbees_ctx* other, double* bc, double* l1);
  * GBEES_ERR_BUFFER. The additions are atomic, so the last bits of p may differ between calls. */
 int gbees_marginal(gbees_ctx* ctx, const int* dims, int m, int32_t* keys, double* p, int64_t cap, int64_t* count);
 
+/* Conservative remap of the PDF onto a grid with origin origin2 [n] and spacing dx2 [n] (host), dx2[j] >= dx[j]
+ * for every j (else GBEES_ERR_ARG). The paper compares runs on grids of different cell width with the eta = 0.5
+ * reference (spatial convergence) without saying how; reading A19: the PDF is piecewise
+ * constant over its cells, and cell d of the target grid receives P_c times the fraction of c's volume inside d
+ * (a product of 1-D overlap fractions; overlaps below 1e-12 of a cell width are dropped). Mass is preserved.
+ * Output as for gbees_marginal: *count target cells in unspecified order, keys [cap*n] int32 row-major (cell
+ * coordinates on the target grid), p [cap]; host or device buffers; keys == NULL or p == NULL: only *count;
+ * cap < *count: GBEES_ERR_BUFFER. Import the result into a context of the target spacing (gbees_import) to
+ * compare it with a run on that grid (gbees_compare). The context is not modified. */
+int gbees_resample(gbees_ctx* ctx, const double* origin2, const double* dx2, int32_t* keys, double* p, int64_t cap, int64_t* count);
+
 /* Write the active cells in unspecified order: keys [cap*n] int32 row-major, p [cap] (normalised).
  * Buffers: host or device (detected), caller-owned. keys == NULL and p == NULL: only *count.
  * cap < count: nothing written, *count = needed, GBEES_ERR_BUFFER. count: host pointer. */

@@ -61,6 +61,7 @@ def lib():
         L.gbees_compare.argtypes = [vp, vp, dp, dp]
         L.gbees_correct_range.argtypes = [vp, dp, C.c_double, C.c_double]
         L.gbees_marginal.argtypes = [vp, C.POINTER(C.c_int), C.c_int, vp, vp, C.c_int64, C.POINTER(C.c_int64)]
+        L.gbees_resample.argtypes = [vp, dp, dp, vp, vp, C.c_int64, C.POINTER(C.c_int64)]
         L.gbees_stats.argtypes = [vp, C.POINTER(Stats)]
         L.gbees_profile.argtypes = [vp, C.c_int, dp, C.POINTER(C.c_int64)]
         L.gbees_last_error.argtypes = [vp]
@@ -165,6 +166,21 @@ class Gbees:
         keys = np.empty((M, len(dims)), dtype=np.int32)
         p = np.empty(M, dtype=np.float64)
         self._chk(lib().gbees_marginal(self._h, d, len(dims), keys.ctypes.data, p.ctypes.data, M, C.byref(cnt)))
+        if sort and M:
+            order = np.lexsort(keys.T[::-1])
+            keys, p = keys[order], p[order]
+        return keys, p
+
+    def resample(self, origin2, dx2, sort=True):
+        """Host conservative remap onto the grid (origin2, dx2): (keys int32 [M, n], p float64 [M])."""
+        _, op = _d(origin2)
+        _, hp = _d(dx2)
+        cnt = C.c_int64()
+        self._chk(lib().gbees_resample(self._h, op, hp, None, None, 0, C.byref(cnt)))
+        M = cnt.value
+        keys = np.empty((M, self.n), dtype=np.int32)
+        p = np.empty(M, dtype=np.float64)
+        self._chk(lib().gbees_resample(self._h, op, hp, keys.ctypes.data, p.ctypes.data, M, C.byref(cnt)))
         if sort and M:
             order = np.lexsort(keys.T[::-1])
             keys, p = keys[order], p[order]

@@ -239,6 +239,11 @@ __global__ void __launch_bounds__(TPB) k_marg_accumulate(GP, const __grid_consta
     ST;
     phase_marg_accumulate<NDIM>(p, st, ds, g, skey, sval);
 }
+template <int NDIM>
+__global__ void __launch_bounds__(TPB) k_resample_accumulate(GP, const __grid_constant__ ResampleArgs g, unsigned long long* skey, double* sval) {
+    ST;
+    phase_resample_accumulate<NDIM>(p, st, ds, g, skey, sval);
+}
 __global__ void __launch_bounds__(TPB) k_marg_emit(DevState* ds, const __grid_constant__ MargArgs g, const unsigned long long* skey,
                                                    const double* sval, int32_t* keys, double* out, unsigned cap) {
     phase_marg_emit(ds, g, skey, sval, keys, out, cap);
@@ -890,6 +895,65 @@ int gbees_marginal(gbees_ctx* c, const int* dims, int m, int32_t* keys, double* 
     if (cap < (int64_t)got) return GBEES_ERR_BUFFER;
     if (!dev_out) {
         CU(cudaMemcpyAsync(keys, dk, (size_t)got * m * 4, cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaMemcpyAsync(pv, dp, (size_t)got * 8, cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+    }
+    return GBEES_OK;
+}
+
+int gbees_resample(gbees_ctx* c, const double* origin2, const double* dx2, int32_t* keys, double* pv, int64_t cap, int64_t* count) {
+    if (!c || !origin2 || !dx2 || !count) return GBEES_ERR_ARG;
+    if (c->sticky) return c->sticky;
+    const int n = c->p.n;
+    ResampleArgs g;
+    std::memset(&g, 0, sizeof(g));
+    for (int j = 0; j < n; ++j) {
+        if (!(dx2[j] >= c->p.h[j])) return GBEES_ERR_ARG;           // the target grid is at least as coarse in every dimension
+        g.o2[j] = origin2[j]; g.h2[j] = dx2[j];
+    }
+    g.mbits = c->p.bits;
+    const unsigned long long N = c->h_st->N;
+    if (N == 0) { *count = 0; return GBEES_OK; }
+    CU(cudaSetDevice(c->device));
+    g.S = 1024;
+    while (g.S < 4 * N) g.S <<= 1;                                // a coarser grid has fewer cells than the source: load factor <= 0.25 + halo
+    const size_t ocap = (size_t)g.S / 2;                           // output rows staged at most (distinct target cells <= slots in use)
+    const size_t need = (size_t)g.S * 16 + ocap * (4 * (size_t)n + 8) + 64;
+    if (need > c->stage_bytes) { c->err = "resample: scratch larger than the staging area"; return GBEES_ERR_CAPACITY; }   // a query: not sticky
+    unsigned long long* skey = reinterpret_cast<unsigned long long*>(c->st.phi);
+    double* sval = reinterpret_cast<double*>(skey + g.S);
+    char* stage = reinterpret_cast<char*>(sval + g.S);
+    auto on_device = [](const void* ptr) {
+        cudaPointerAttributes a;
+        if (cudaPointerGetAttributes(&a, ptr) != cudaSuccess) { cudaGetLastError(); return false; }
+        return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+    };
+    const bool dev_out = keys && pv && on_device(keys) && on_device(pv);
+    const unsigned ucap = keys && pv ? (dev_out ? (unsigned)(cap < (int64_t)ocap ? cap : (int64_t)ocap) : (unsigned)ocap) : 0u;
+    const size_t kbytes = (ocap * n * 4 + 7) & ~(size_t)7;
+    int32_t* dk = dev_out ? keys : reinterpret_cast<int32_t*>(stage);
+    double* dp = dev_out ? pv : reinterpret_cast<double*>(stage + kbytes);
+    MargArgs e;                                                    // emit: all n target coordinates, in order
+    std::memset(&e, 0, sizeof(e));
+    e.m = n; e.mbits = g.mbits; e.S = g.S;
+    CU(cudaMemsetAsync(&c->d_st->export_count, 0, sizeof(unsigned), c->stream));
+    k_marg_clear<<<c->grid, TPB, 0, c->stream>>>(skey, sval, g.S);
+    dispatch_n(c, [&](auto N_) {
+        k_resample_accumulate<decltype(N_)::value><<<c->grid, TPB, 0, c->stream>>>(c->p, c->st, c->d_st, g, skey, sval);
+        return GBEES_OK;
+    });
+    k_marg_emit<<<c->grid, TPB, 0, c->stream>>>(c->d_st, e, skey, sval, dk, dp, ucap);
+    c->launches += 3;
+    CU(cudaGetLastError());
+    unsigned got = 0;
+    CU(cudaMemcpyAsync(&got, &c->d_st->export_count, sizeof(unsigned), cudaMemcpyDeviceToHost, c->stream));
+    int rc = sync_state(c);                                        // table-full / finer-grid faults raised on the device
+    if (rc) return rc;
+    *count = got;
+    if (!keys || !pv) return GBEES_OK;                            // count only
+    if (cap < (int64_t)got || got > ucap) return GBEES_ERR_BUFFER;
+    if (!dev_out) {
+        CU(cudaMemcpyAsync(keys, dk, (size_t)got * n * 4, cudaMemcpyDeviceToHost, c->stream));
         CU(cudaMemcpyAsync(pv, dp, (size_t)got * 8, cudaMemcpyDeviceToHost, c->stream));
         CU(cudaStreamSynchronize(c->stream));
     }

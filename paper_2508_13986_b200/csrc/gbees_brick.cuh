@@ -1181,6 +1181,82 @@ __device__ __forceinline__ void phase_marg_emit(DevState* ds, const MargArgs& g,
     }
 }
 
+// f1, spatial convergence: conservative remap of the PDF onto a grid of another origin / spacing
+// (reading A19: the PDF is piecewise constant over its cells; cell d of the other grid receives P_c times the
+// overlap volume fraction, a product of 1-D overlap fractions). The target grid is at least as coarse in every
+// dimension, so a cell overlaps at most two target cells per dimension. Same scratch table as the marginals.
+// The integer decisions (which target cells, sliver cut-off) use the arithmetic of oracle/resample_oracle.py.
+struct ResampleArgs {
+    double o2[MAXN], h2[MAXN];
+    int mbits;
+    unsigned long long S;
+};
+template <int NDIM>
+__device__ void phase_resample_accumulate(const Params& p, const Store& st, DevState* ds, const ResampleArgs& g,
+                                          unsigned long long* skey, double* sval) {
+    const uint32_t NB = min(ds->NB, p.capB);
+    const uint64_t items = (uint64_t)NB * 64;
+    const double scale = ds->scale;
+    const long long mbias = 1ll << (g.mbits - 1);
+    for (uint64_t i = gtid(); i < items; i += gthreads()) {
+        const uint32_t b = (uint32_t)(i >> 6);
+        const int l = (int)(i & 63);
+        if (!((st.mask[b] >> l) & 1ull)) continue;
+        int32_t B[NDIM], c[NDIM];
+        unpack<NDIM>(p, st.bkey[b], B);
+        cell_coords<NDIM>(B, l, c);
+        const double pc = scale * st.Q[i];
+        long long d0[NDIM];
+        double w[NDIM][2];
+        int cnt[NDIM];
+#pragma unroll
+        for (int j = 0; j < NDIM; ++j) {
+            const double h = p.h[j], o2 = g.o2[j], h2 = g.h2[j];
+            const double lo = DADD(p.mu[j], DMUL((double)c[j] - 0.5, h)), hi = DADD(p.mu[j], DMUL((double)c[j] + 0.5, h));
+            const long long dl = (long long)floor(DADD(__ddiv_rn(DSUB(lo, o2), h2), 0.5));
+            const long long dh = (long long)floor(DADD(__ddiv_rn(DSUB(hi, o2), h2), 0.5));
+            if (dh > dl + 1) atomicOr(&ds->err, E_DEGENERATE);      // target grid finer than the source (rejected by the host)
+            int n_ = 0;
+            long long first = dl;
+            for (int k = 0; k < 2; ++k) {
+                const long long d = dl + k;
+                if (d > dh) break;
+                const double a = fmax(lo, DADD(o2, DMUL((double)d - 0.5, h2))), e = fmin(hi, DADD(o2, DMUL((double)d + 0.5, h2)));
+                if (DSUB(e, a) > DMUL(1e-12, h)) {
+                    if (n_ == 0) first = d;
+                    w[j][n_++] = __ddiv_rn(DSUB(e, a), h);
+                }
+            }
+            // target coordinates must fit the key fields of the scratch table (the width of the grid's own fields)
+            if (first < -mbias || first + 1 > mbias - 1) { atomicOr(&ds->err, E_KEY_RANGE); n_ = 0; }
+            d0[j] = first; cnt[j] = n_;                              // the (at most two) target cells are consecutive
+            if (n_ < 2) w[j][1] = 0.0;
+            if (n_ < 1) w[j][0] = 0.0;
+        }
+        for (int combo = 0; combo < (1 << NDIM); ++combo) {
+            double wt = 1.0;
+            unsigned long long key = 0ull;
+            bool ok = true;
+#pragma unroll
+            for (int j = 0; j < NDIM; ++j) {
+                const int k = (combo >> j) & 1;
+                ok = ok && k < cnt[j];
+                wt = DMUL(wt, k ? w[j][1] : w[j][0]);
+                key = (key << g.mbits) | (unsigned long long)(d0[j] + k + mbias);
+            }
+            if (!ok) continue;
+            unsigned long long s = home_slot(key, g.S);
+            for (unsigned long long tries = 0;; ++tries) {
+                if (tries == g.S) { atomicOr(&ds->err, E_TABLE_FULL); break; }
+                unsigned long long cur = *reinterpret_cast<volatile unsigned long long*>(&skey[s]);
+                if (cur == KEY_EMPTY) cur = atomicCAS(&skey[s], KEY_EMPTY, key);
+                if (cur == KEY_EMPTY || cur == key) { atomicAdd(&sval[s], DMUL(pc, wt)); break; }
+                if (++s == g.S) s = 0;
+            }
+        }
+    }
+}
+
 // export: a warp reserves popc(mask) output rows per brick (order of bricks is unspecified)
 template <int NDIM>
 __device__ void phase_export(const Params& p, const Store& st, DevState* ds, int32_t* keys, double* out) {

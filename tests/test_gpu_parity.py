@@ -484,6 +484,72 @@ def test_compare_metrics_and_temporal_convergence():
     print("temporal convergence, E(eps = 1, 0.5, 0.2) vs eps = 0.02:", errs)
 
 
+def test_resample_parity_and_spatial_convergence():
+    """f1, spatial half: runs with cell width eta * h*, eta = 1.25, 1, 0.8, 0.6, against the
+    eta = 0.5 reference at C = 0.1. The reference is remapped conservatively onto each coarser grid
+    (gbees_resample, reading A19), imported into a context of that spacing and compared with gbees_compare.
+    Checked: the remap against oracle/resample_oracle.py cell by cell (same key set, masses 1e-12), mass
+    preserved; BC and E against the metrics oracle applied to the ORACLE's runs; E falls and BC rises as
+    eta falls."""
+    from oracle import metrics_oracle as M, resample_oracle as RO
+    cfg = W.config0()
+    hstar, t_end, n = 0.5, 0.02, 3
+    mean = np.asarray(cfg["mean"], dtype=np.float64)
+
+    def setup(eta):
+        dx = [eta * hstar] * n
+        thr = cfg["thresh"] * eta ** n                              # the same density threshold on every grid
+        return dx, thr
+
+    def run_gpu(eta):
+        dx, thr = setup(eta)
+        g = G(n, dx, thr, cfg["dyn"], cfg["params"], cfl=0.1, max_cells=1 << 19)
+        g.init_gaussian(mean, cfg["cov"])
+        g.run(t_end, prune_every=1)
+        assert g.time() == t_end
+        return g
+
+    def run_oracle(eta):
+        dx, thr = setup(eta)
+        o = Oracle(n, dx, thr, cfg["dyn"], cfg["params"], cfl=0.1)
+        o.init_gaussian(mean, cfg["cov"])
+        while o.time() < t_end:
+            o.step(t_end - o.time()); o.prune()
+        return o.export()
+
+    ref = run_gpu(0.5)
+    rk, rp = ref.export()
+    ork, orp = run_oracle(0.5)
+    assert np.array_equal(rk, ork)
+    errs, bcs = [], []
+    for eta in (1.25, 1.0, 0.8, 0.6):
+        dx, thr = setup(eta)
+        # the remap itself: GPU on the GPU's reference state vs the oracle remap of the same state
+        gk, gp = ref.resample(mean, dx)
+        wk, wp = RO.resample(rk, rp, mean, [0.5 * hstar] * n, mean, dx)
+        assert np.array_equal(gk, wk), f"eta {eta}: remapped key sets differ"
+        assert np.max(np.abs(gp - wp)) <= 1e-12 * np.max(np.abs(wp))
+        assert gp.sum() == pytest.approx(rp.sum(), rel=1e-12)        # mass preserved
+        # metrics on the coarse grid
+        g = run_gpu(eta)
+        tmp = G(n, dx, thr, cfg["dyn"], cfg["params"], cfl=0.1, max_cells=1 << 19)
+        tmp.import_state(mean, gk, gp)
+        bc, l1 = g.compare(tmp)
+        ok2, op2 = run_oracle(eta)
+        obc, ol1 = M.bc_and_l1(ok2, op2, *RO.resample(ork, orp, mean, [0.5 * hstar] * n, mean, dx))
+        assert bc == pytest.approx(obc, abs=1e-8) and l1 == pytest.approx(ol1, abs=1e-8)
+        errs.append(l1); bcs.append(bc)
+        tmp.close(); g.close()
+    assert errs[0] > errs[1] > errs[2] > errs[3] > 0.0               # E(eta) falls with the cell width
+    assert bcs[0] < bcs[1] < bcs[2] < bcs[3] <= 1.0 + 1e-6
+    # argument checks: a finer target grid is refused; the same grid is the identity
+    with pytest.raises(Exception):
+        ref.resample(mean, [0.1] * n)
+    ik, ip = ref.resample(mean, [0.5 * hstar] * n)
+    assert np.array_equal(ik, rk) and np.allclose(ip, rp, rtol=1e-14, atol=0)
+    print("spatial convergence, E(eta = 1.25, 1, 0.8, 0.6) vs eta = 0.5:", errs, "BC:", bcs)
+
+
 def test_marginals_of_the_6d_pdf():
     """f3: the two 3-D marginals of the 6-D Lorenz '96 PDF (and a 1-D, a 2-D one with
     permuted dimensions) by device hash-accumulation against the numpy group-by of the exported state."""
