@@ -52,7 +52,10 @@ typedef struct gbees_opts {
     int limiter;         /* 0 = monotonised central, 1 = none (phi == 1, test mode) */
     int no_grow;         /* test mode: gbees_step does not grow the grid */
     int no_normalise;    /* test mode: keep raw (un-normalised) masses after step / prune */
-    int run_mode;        /* gbees_run: 0 = device-side step control, no host round trip per step (default); 1 = host loop of gbees_step / gbees_prune */
+    int run_mode;        /* gbees_run: 0 = device-side step control, no host round trip per step (default); 1 = host loop of gbees_step /
+                            gbees_prune; 2 = as 0 with the chunks of steps captured as a CUDA graph; 3 = one cooperative launch over
+                            the whole GPU with grid barriers between the phases. 2 and 3 are kept for measurement:
+                            same results, 0 is the fastest */
     int device;          /* CUDA device ordinal */
     void* stream;        /* cudaStream_t to run on (e.g. torch's current stream); NULL = default */
 } gbees_opts;

@@ -135,14 +135,23 @@ __global__ void k_after_compact(const __grid_constant__ Params p, DevState* ds) 
 // (barrier.cluster, which also invalidates L1) separates the phases instead of kernel boundaries.
 // Same phases, same order, same arithmetic as the stream of launches; leaves the loop when the run
 // is over or the grid has outgrown the cluster (the host then goes on with the launches).
-template <int NDIM, int DYN, bool FAST>
+// GRID = true is the same loop for grids of any size as ONE cooperative launch that fills the GPU, with
+// grid-wide barriers between the phases: the paper's own execution model. It is kept as
+// opts.run_mode = 3 for measurement; the stream of launches is faster.
+template <int NDIM, int DYN, bool FAST, bool GRID>
 __global__ void __launch_bounds__(TPB) k_run_small(GP, int prune_every, int no_grow, unsigned long long k_start, uint32_t nb_limit) {
     namespace cg = cooperative_groups;
-    cg::cluster_group cl = cg::this_cluster();
+    struct Barrier {
+        __device__ void sync() const {
+            if constexpr (GRID) cg::this_grid().sync();
+            else cg::this_cluster().sync();
+        }
+    } cl;
     __shared__ bool s_last;
     unsigned long long k = k_start;
     for (;;) {
         cl.sync();
+        if (GRID && (double)ds->NB_before_grow > p.load_factor * (double)ds->slots && ds->slots < p.slots) break;   // the host rehashes
         // uniform: go and NB_before_grow (= NB at the top of the loop) are written by begin_step only, i.e.
         // before this barrier; NB itself is bumped by the grow below and must not be tested here
         if (!ds->go || ds->NB_before_grow > nb_limit) break;
@@ -276,6 +285,10 @@ struct gbees_ctx {
     int run_mode = 0;            // 0 = device-side step control, 1 = host loop over step/prune
     int small_ok = 1;            // the single-cluster persistent loop can be launched on this device
     int pdl = 1;                 // programmatic dependent launch between the kernels of a step / prune
+    cudaGraphExec_t graph_exec = nullptr;   // run_mode 2: the captured chunk
+    int64_t graph_chunk = 0;
+    int graph_prune = 0;
+    int64_t graph_launches = 0;
     int run_blocks_per_sm = 0;
     int64_t n_inserted = 0, n_pruned = 0;
     std::string err;
@@ -481,6 +494,7 @@ int gbees_destroy(gbees_ctx* c) {
     cudaStreamSynchronize(c->stream);
     drain_events(c);
     for (cudaEvent_t e : c->ev_free) cudaEventDestroy(e);
+    if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
     for (int i = 0; i < c->nallocs; ++i) cudaFree(c->allocs[i]);
     if (c->h_st) cudaFreeHost(c->h_st);
     delete c;
@@ -1000,7 +1014,7 @@ static int launch_small(gbees_ctx* c, int prune_every, unsigned long long k_star
         constexpr int NN = decltype(N_)::value, DD = decltype(D_)::value;
         constexpr size_t smem = sizeof(Flux1Smem<NN>) * WPB;
         const bool fast = c->p.hi_res && !c->p.limiter;
-        auto kern = fast ? k_run_small<NN, DD, true> : k_run_small<NN, DD, false>;
+        auto kern = fast ? k_run_small<NN, DD, true, false> : k_run_small<NN, DD, false, false>;
         if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return GBEES_ERR_CUDA;
         cudaLaunchConfig_t cfg = {};
         cfg.gridDim = dim3(8); cfg.blockDim = dim3(TPB); cfg.dynamicSmemBytes = smem; cfg.stream = c->stream;
@@ -1016,6 +1030,55 @@ static int launch_small(gbees_ctx* c, int prune_every, unsigned long long k_star
     });
     if (rc == GBEES_ERR_CUDA) { cudaGetLastError(); c->small_ok = 0; }   // not launchable here: use the launches
     return rc;
+}
+
+// opts.run_mode = 3: the whole loop as one cooperative launch over the GPU (measurement; see k_run_small)
+static int launch_coop(gbees_ctx* c, int prune_every, unsigned long long k_start) {
+    return dispatch(c, [&](auto N_, auto D_) {
+        constexpr int NN = decltype(N_)::value, DD = decltype(D_)::value;
+        constexpr size_t smem = sizeof(Flux1Smem<NN>) * WPB;
+        const bool fast = c->p.hi_res && !c->p.limiter;
+        auto kern = fast ? k_run_small<NN, DD, true, true> : k_run_small<NN, DD, false, true>;
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return GBEES_ERR_CUDA;
+        int per_sm = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, TPB, smem) != cudaSuccess || per_sm < 1) return GBEES_ERR_CUDA;
+        Params p = c->p; Store st = c->st; DevState* ds = c->d_st;
+        int pe = prune_every, ng = c->no_grow; unsigned long long ks = k_start; uint32_t lim = c->p.capB;
+        void* args[] = {&p, &st, &ds, &pe, &ng, &ks, &lim};
+        cudaError_t e = cudaSuccess;
+        phase(c, GBEES_PH_RUN, 1, [&] {
+            e = cudaLaunchCooperativeKernel((const void*)kern, dim3((unsigned)(per_sm * c->sms)), dim3(TPB), args, smem, c->stream);
+        });
+        return e == cudaSuccess ? GBEES_OK : GBEES_ERR_CUDA;
+    });
+}
+
+// opts.run_mode = 2: a chunk of steps (+ its prunes) captured once as a CUDA graph and relaunched (measurement).
+// The launches are identical from chunk to chunk -- all state is on the device -- as long as the chunk is a
+// multiple of the prune cadence.
+static int enqueue_step(gbees_ctx* c);
+static int enqueue_prune(gbees_ctx* c);
+static int launch_graph_chunk(gbees_ctx* c, int64_t chunk, int prune_every) {
+    if (!c->graph_exec || c->graph_chunk != chunk || c->graph_prune != prune_every) {
+        if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+        cudaGraph_t g = nullptr;
+        const int64_t l0 = c->launches;
+        if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) return GBEES_ERR_CUDA;
+        int rc = GBEES_OK;
+        for (int64_t i = 1; i <= chunk && !rc; ++i) {
+            rc = enqueue_step(c);
+            if (!rc && prune_every > 0 && i % prune_every == 0) rc = enqueue_prune(c);
+        }
+        if (cudaStreamEndCapture(c->stream, &g) != cudaSuccess || rc) { if (g) cudaGraphDestroy(g); return rc ? rc : GBEES_ERR_CUDA; }
+        const cudaError_t e = cudaGraphInstantiate(&c->graph_exec, g, 0);
+        cudaGraphDestroy(g);
+        if (e != cudaSuccess) { c->graph_exec = nullptr; return GBEES_ERR_CUDA; }
+        c->graph_chunk = chunk; c->graph_prune = prune_every;
+        c->graph_launches = c->launches - l0;
+        c->launches = l0;
+    }
+    c->launches += c->graph_launches;
+    return cudaGraphLaunch(c->graph_exec, c->stream) == cudaSuccess ? GBEES_OK : GBEES_ERR_CUDA;
 }
 
 // host loop over gbees_step / gbees_prune with a host round trip per call (opts.run_mode = 1)
@@ -1060,6 +1123,27 @@ int gbees_run(gbees_ctx* c, double t_target, int64_t max_steps, int prune_every,
                 if (c->h_st->NB <= SMALL_NB_ENTER) c->small_ok = 0;   // left the loop for another reason: do not spin
                 else continue;
             } else if (lrc != GBEES_ERR_CUDA) return fail(c, lrc, "unsupported (n, dynamics) pair");
+        }
+        if (c->run_mode == 3 && !c->profile) {               // one cooperative launch runs until the end (or a rehash)
+            const int lrc = launch_coop(c, prune_every, (unsigned long long)k);
+            if (lrc != GBEES_OK) return fail(c, lrc, "cooperative launch failed");
+            if ((rc = sync_state(c))) break;
+            if ((rc = rehash_if_needed(c))) break;
+            k = (int64_t)(c->h_st->steps - steps0);
+            if (!c->h_st->go || k >= max_steps) break;
+            continue;
+        }
+        if (c->run_mode == 2 && !c->profile && (prune_every <= 0 || k % prune_every == 0)) {
+            const int64_t gchunk = prune_every > 0 ? (int64_t)prune_every * ((16 + prune_every - 1) / prune_every) : 16;
+            if (gchunk <= max_steps - k) {
+                if ((rc = launch_graph_chunk(c, gchunk, prune_every)))
+                    return fail(c, rc, std::string("CUDA graph of a chunk of steps (not capturable on the legacy default stream): ") + cudaGetErrorString(cudaGetLastError()));
+                k += gchunk;
+                if ((rc = sync_state(c))) break;
+                if ((rc = rehash_if_needed(c))) break;
+                if (!c->h_st->go || k >= max_steps) break;
+                continue;
+            }
         }
         int64_t chunk = 16;
         if (c->h_st->dt > 0.0 && t_target < 1e299) {     // do not enqueue far past the expected end

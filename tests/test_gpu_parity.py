@@ -207,6 +207,26 @@ def test_run_persistent_loop_lorenz96_to_time(prune_every):
     compare_states(*g.export(), *o.export(), cfg["thresh"], 1e-9, what="L96 run + step + prune")
 
 
+@pytest.mark.parametrize("run_mode", [2, 3])
+def test_run_modes_graph_and_cooperative_are_observationally_identical(run_mode):
+    """a9: gbees_run with the chunks of steps captured as a CUDA graph (run_mode 2) and as
+    ONE cooperative launch over the whole GPU with grid barriers between the phases (run_mode 3, the paper's
+    execution model) gives the oracle's step / prune sequence, like the default stream of launches."""
+    import torch
+    cfg = W.config2()
+    cfg.update(thresh=1e-5, max_cells=1 << 20)
+    stream = torch.cuda.Stream()                                   # (a graph cannot be captured on the legacy default stream)
+    g = G(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfg["cfl"], max_cells=cfg["max_cells"],
+          run_mode=run_mode, stream=stream.cuda_stream)
+    g.init_gaussian(cfg["mean"], cfg["cov"])
+    o, k = oracle_run(cfg, t_end=0.2)
+    assert k > 20                                                   # more than one graph chunk
+    assert g.run(0.2, prune_every=cfg["prune_every"]) == k
+    assert g.time() == o.time() == 0.2
+    compare_states(*g.export(), *o.export(), cfg["thresh"], 1e-9, what=f"run_mode {run_mode}")
+    assert g.stats()["steps"] == k and g.stats()["prunes"] == k // cfg["prune_every"]
+
+
 def test_config2_full_size_against_oracle_golden():
     """BASELINE config 2 at full size, in the launch configuration bench.py times (gbees_run, device-side
     step control): step count, final time, cell counts after every 5th step and the masses of 128
