@@ -1185,7 +1185,7 @@ __device__ __forceinline__ void phase_marg_emit(DevState* ds, const MargArgs& g,
 // (reading A19: the PDF is piecewise constant over its cells; cell d of the other grid receives P_c times the
 // overlap volume fraction, a product of 1-D overlap fractions). The target grid is at least as coarse in every
 // dimension, so a cell overlaps at most two target cells per dimension. Same scratch table as the marginals.
-// The integer decisions (which target cells, sliver cut-off) use the arithmetic of oracle/resample_oracle.py.
+// The integer decisions (which target cells, sliver cut-off) follow the operation order DESIGN.md A19 fixes.
 struct ResampleArgs {
     double o2[MAXN], h2[MAXN];
     int mbits;
