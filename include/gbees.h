@@ -58,6 +58,10 @@ typedef struct gbees_opts {
                             same results, 0 is the fastest */
     int device;          /* CUDA device ordinal */
     void* stream;        /* cudaStream_t to run on (e.g. torch's current stream); NULL = default */
+    void* arena;         /* optional caller-owned DEVICE memory (e.g. the data_ptr of a torch uint8 tensor on opts.device) that all
+                            fixed-capacity device structures are carved from instead of cudaMalloc; must stay alive until gbees_destroy,
+                            which does not free it; NULL = the library allocates (capacity is fixed at creation) */
+    int64_t arena_bytes; /* its size; gbees_arena_bytes() says how much gbees_create needs (GBEES_ERR_CAPACITY if too small) */
 } gbees_opts;
 
 typedef struct gbees_stats_t {
@@ -94,6 +98,9 @@ enum {
 
 /* Fill *opts with the defaults (max_cells = 1<<20, load_factor 0.5, cfl 0.9, hi_res 1, MC). */
 int gbees_default_opts(gbees_opts* opts /*host*/);
+/* Device bytes that gbees_create(n, ..., opts) carves from opts->arena (a function of n, max_cells and load_factor
+ * only; opts == NULL: the defaults). bytes: host. */
+int gbees_arena_bytes(int n, const gbees_opts* opts /*host, nullable*/, int64_t* bytes);
 
 /* Allocate all fixed-capacity device structures. dx, params: host, copied.
  * n in [1,6]; n_params must match dynamics_id. opts may be NULL (defaults). */

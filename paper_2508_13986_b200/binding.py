@@ -20,7 +20,7 @@ class GbeesError(RuntimeError):
 class Opts(C.Structure):
     _fields_ = [("max_cells", C.c_int64), ("load_factor", C.c_double), ("cfl", C.c_double),
                 ("hi_res", C.c_int), ("limiter", C.c_int), ("no_grow", C.c_int), ("no_normalise", C.c_int),
-                ("run_mode", C.c_int), ("device", C.c_int), ("stream", C.c_void_p)]
+                ("run_mode", C.c_int), ("device", C.c_int), ("stream", C.c_void_p), ("arena", C.c_void_p), ("arena_bytes", C.c_int64)]
 
 
 class Stats(C.Structure):
@@ -30,6 +30,18 @@ class Stats(C.Structure):
                 ("cells_inserted", C.c_int64), ("cells_prune_scanned", C.c_int64), ("prunes", C.c_int64)]
 
 PHASES = ["grow", "link", "passA", "passB", "mark", "compact", "rebuild", "relink", "sum", "correct", "run"]
+
+
+def arena_bytes(n, max_cells=1 << 20, load_factor=0.5):
+    """Device bytes a context of this capacity carves from a caller-provided arena (gbees_arena_bytes)."""
+    o = Opts()
+    lib().gbees_default_opts(C.byref(o))
+    o.max_cells, o.load_factor = int(max_cells), float(load_factor)
+    b = C.c_int64()
+    rc = lib().gbees_arena_bytes(int(n), C.byref(o), C.byref(b))
+    if rc:
+        raise GbeesError(rc, "gbees_arena_bytes failed")
+    return b.value
 
 
 def lib_path():
@@ -46,6 +58,7 @@ def lib():
         L = C.CDLL(_LIB_PATH)
         vp, dp, ip = C.c_void_p, C.POINTER(C.c_double), C.c_void_p
         L.gbees_default_opts.argtypes = [C.POINTER(Opts)]
+        L.gbees_arena_bytes.argtypes = [C.c_int, C.POINTER(Opts), C.POINTER(C.c_int64)]
         L.gbees_create.argtypes = [C.POINTER(vp), C.c_int, dp, C.c_double, C.c_int, dp, C.c_int, C.POINTER(Opts)]
         L.gbees_destroy.argtypes = [vp]
         L.gbees_init_gaussian.argtypes = [vp, dp, dp]
@@ -80,7 +93,7 @@ class Gbees:
     """One GBEES context on one GPU. Methods mirror the C ABI one to one."""
 
     def __init__(self, n, dx, threshold, dynamics_id, params, max_cells=1 << 20, load_factor=0.5, cfl=0.9,
-                 hi_res=1, limiter=0, no_grow=False, no_normalise=False, run_mode=0, device=0, stream=None):
+                 hi_res=1, limiter=0, no_grow=False, no_normalise=False, run_mode=0, device=0, stream=None, arena=None):
         L = lib()
         self.n = int(n)
         o = Opts()
@@ -90,6 +103,9 @@ class Gbees:
         o.device = int(device)
         o.run_mode = int(run_mode)
         o.stream = C.c_void_p(stream) if stream else None
+        if arena is not None:                       # a torch CUDA uint8 tensor owned by the caller: all device structures live in it
+            o.arena, o.arena_bytes = C.c_void_p(arena.data_ptr()), int(arena.numel() * arena.element_size())
+            self._arena = arena
         self._h = C.c_void_p()
         _, dxp = _d(dx)
         par, pp = _d(params)

@@ -478,6 +478,41 @@ int reset_grid(gbees_ctx* c) {
 // ================================================================================================
 extern "C" {
 
+// brick and table capacity for (max_cells, load_factor): shared by gbees_create and gbees_arena_bytes
+static void plan_capacity(const gbees_opts& o, uint32_t* capB, uint64_t* slots) {
+    uint64_t cb = ((uint64_t)o.max_cells + 15) / 16;     // rows of 64 slots; sized for a fill factor >= 1/16
+    if (cb < 256) cb = 256;
+    *capB = (uint32_t)cb;
+    uint64_t s = (uint64_t)std::ceil((double)cb / o.load_factor);
+    if (s < (1ull << 16)) s = 1ull << 16;
+    *slots = s;
+}
+constexpr unsigned GRID_MAX = 4096;     // upper bound of c->grid (8 blocks x SMs) used to size the partial-sum array
+// device bytes of every fixed-capacity structure, in allocation order (each rounded up to 256 bytes)
+static size_t plan_bytes(int n, uint32_t capB, uint64_t slots, size_t* sizes /*[21]*/) {
+    const size_t cb = capB, nd = 2 * (size_t)n, ntiles = (capB + SCAN_TILE - 1) / SCAN_TILE;
+    const size_t raw[21] = {cb * 512, cb * 512, cb * nd * 32 * 8, cb * 8, cb * 8, cb * 8, cb * 8, cb * 64 * 2, cb * nd * 4,
+                            cb * 4, cb * 4, cb * 8, slots * sizeof(ulonglong2), slots * 8, cb * 8, cb * 8, cb * 8, cb * 4,
+                            (ntiles + 1) * 8, (size_t)GRID_MAX * 8, sizeof(DevState)};
+    size_t tot = 0;
+    for (int i = 0; i < 21; ++i) { sizes[i] = (raw[i] + 255) & ~(size_t)255; tot += sizes[i]; }
+    return tot;
+}
+
+int gbees_arena_bytes(int n, const gbees_opts* opts_in, int64_t* bytes) {
+    if (!bytes || n < 1 || n > MAXN) return GBEES_ERR_ARG;
+    gbees_opts o;
+    gbees_default_opts(&o);
+    if (opts_in) o = *opts_in;
+    if (o.max_cells <= 0) o.max_cells = 1 << 20;
+    if (!(o.load_factor > 0.0 && o.load_factor < 1.0)) o.load_factor = 0.5;
+    if (o.max_cells >= (int64_t)1 << 32) return GBEES_ERR_ARG;
+    uint32_t capB; uint64_t slots; size_t sizes[21];
+    plan_capacity(o, &capB, &slots);
+    *bytes = (int64_t)plan_bytes(n, capB, slots, sizes) + 256;    // + alignment slack of the arena's base
+    return GBEES_OK;
+}
+
 int gbees_default_opts(gbees_opts* o) {
     if (!o) return GBEES_ERR_ARG;
     std::memset(o, 0, sizeof(*o));
@@ -538,13 +573,7 @@ int gbees_create(gbees_ctx** out, int n, const double* dx, double threshold, int
     for (int k = 0; k < need; ++k) p.par[k] = params[k];
     p.thresh = threshold; p.cfl = o.cfl;
     p.max_cells = (uint64_t)o.max_cells;
-    {   // brick capacity: rows of 64 slots; sized for a fill factor >= 1/16
-        uint64_t cb = ((uint64_t)o.max_cells + 15) / 16;
-        if (cb < 256) cb = 256;
-        p.capB = (uint32_t)cb;
-    }
-    p.slots = (uint64_t)std::ceil((double)p.capB / o.load_factor);
-    if (p.slots < (1ull << 16)) p.slots = 1ull << 16;
+    plan_capacity(o, &p.capB, &p.slots);
     p.load_factor = o.load_factor;
 
     auto bail = [&](int code, const std::string& m) { fprintf(stderr, "gbees_create: %s\n", m.c_str()); gbees_destroy(c); return code; };
@@ -567,22 +596,28 @@ int gbees_create(gbees_ctx** out, int n, const double* dx, double threshold, int
         }) != GBEES_OK)
         return bail(GBEES_ERR_CUDA, "unsupported (n, dynamics) pair or shared-memory opt-in failed");
     const size_t cb = p.capB, nd = 2 * (size_t)n;
-    auto alloc = [&](void** ptr, size_t bytes) {
-        cudaError_t e2 = cudaMalloc(ptr, bytes);
-        if (e2 == cudaSuccess) c->allocs[c->nallocs++] = *ptr;
-        return e2;
-    };
+    // all fixed-capacity structures: from the caller's arena (opts.arena, carved in 256-byte units) or cudaMalloc
     Store& st = c->st;
     c->stage_bytes = cb * nd * 32 * 8;
-    if (alloc((void**)&st.Q, cb * 512) || alloc((void**)&st.Qn, cb * 512) || alloc((void**)&st.phi, c->stage_bytes) ||
-        alloc((void**)&st.bkey, cb * 8) || alloc((void**)&st.mask, cb * 8) || alloc((void**)&st.grown, cb * 8) ||
-        alloc((void**)&st.keep, cb * 8) || alloc((void**)&st.fetch, cb * 64 * 2) || alloc((void**)&st.adj, cb * nd * 4) ||
-        alloc((void**)&st.slot_of, cb * 4) || alloc((void**)&st.slist, cb * 4) || alloc((void**)&st.smask, cb * 8) || alloc((void**)&st.table, p.slots * sizeof(ulonglong2)) ||
-        alloc((void**)&st.pend, p.slots * 8) || alloc((void**)&st.bkey2, cb * 8) || alloc((void**)&st.mask2, cb * 8) ||
-        alloc((void**)&st.grown2, cb * 8) || alloc((void**)&st.newrow, cb * 4) ||
-        alloc((void**)&st.tile_state, (size_t)(c->ntiles_max + 1) * 8) || alloc((void**)&st.partial, (size_t)c->grid * 8) ||
-        alloc((void**)&c->d_st, sizeof(DevState)))
-        return bail(GBEES_ERR_CUDA, std::string("cudaMalloc: ") + cudaGetErrorString(cudaGetLastError()));
+    size_t sizes[21];
+    const size_t total = plan_bytes(n, p.capB, p.slots, sizes);
+    if ((size_t)c->grid > GRID_MAX) return bail(GBEES_ERR_ARG, "more SMs than the partial-sum array is planned for");
+    void** const ptrs[21] = {(void**)&st.Q, (void**)&st.Qn, (void**)&st.phi, (void**)&st.bkey, (void**)&st.mask, (void**)&st.grown,
+                             (void**)&st.keep, (void**)&st.fetch, (void**)&st.adj, (void**)&st.slot_of, (void**)&st.slist, (void**)&st.smask,
+                             (void**)&st.table, (void**)&st.pend, (void**)&st.bkey2, (void**)&st.mask2, (void**)&st.grown2, (void**)&st.newrow,
+                             (void**)&st.tile_state, (void**)&st.partial, (void**)&c->d_st};
+    if (o.arena) {
+        char* base = reinterpret_cast<char*>((reinterpret_cast<uintptr_t>(o.arena) + 255) & ~(uintptr_t)255);
+        if (o.arena_bytes < (int64_t)(total + (size_t)(base - reinterpret_cast<char*>(o.arena))))
+            return bail(GBEES_ERR_CAPACITY, "opts.arena is smaller than gbees_arena_bytes()");
+        for (int i = 0; i < 21; ++i) { *ptrs[i] = base; base += sizes[i]; }
+    } else {
+        for (int i = 0; i < 21; ++i) {
+            if (cudaMalloc(ptrs[i], sizes[i]) != cudaSuccess)
+                return bail(GBEES_ERR_CUDA, std::string("cudaMalloc: ") + cudaGetErrorString(cudaGetLastError()));
+            c->allocs[c->nallocs++] = *ptrs[i];
+        }
+    }
     if (cudaMallocHost((void**)&c->h_st, sizeof(DevState)) != cudaSuccess) return bail(GBEES_ERR_CUDA, "cudaMallocHost");
     cudaMemsetAsync(st.Q, 0, cb * 512, c->stream);
     cudaMemsetAsync(st.Qn, 0, cb * 512, c->stream);

@@ -37,6 +37,19 @@ def test_default_opts_and_argument_checks_without_gpu():
     assert L.gbees_create(ctypes.byref(h), 3, dx, 1e-5, 0, par, 2, None) == -1      # too few params
 
 
+def test_arena_bytes_without_gpu():
+    """caller-provided device arena; its size is a host-side function of (n, max_cells, load_factor)."""
+    from paper_2508_13986_b200 import binding
+    small, big = binding.arena_bytes(6, 1 << 16), binding.arena_bytes(6, 1 << 22)
+    assert 0 < small < big
+    # dominated by the bricks: 2 x 512 (Q, Qn) + 2n x 256 (phi) bytes per brick, max_cells / 16 bricks
+    bricks = (1 << 22) // 16
+    assert big >= bricks * (1024 + 12 * 256) and big < 2 * bricks * (1024 + 12 * 256)
+    assert binding.arena_bytes(3, 1 << 22) < big                       # fewer faces per brick
+    b = ctypes.c_int64()
+    assert binding.lib().gbees_arena_bytes(7, None, ctypes.byref(b)) == -1
+
+
 def test_product_does_not_import_oracle():
     pkg = os.path.join(ROOT, "paper_2508_13986_b200")
     for dirpath, _, files in os.walk(pkg):

@@ -570,6 +570,30 @@ def test_resample_parity_and_spatial_convergence():
     print("spatial convergence, E(eta = 1.25, 1, 0.8, 0.6) vs eta = 0.5:", errs, "BC:", bcs)
 
 
+def test_caller_provided_device_arena():
+    """every fixed-capacity device structure is carved from a caller-owned torch tensor
+    (opts.arena) instead of cudaMalloc; same results; an arena that is too small is refused."""
+    import torch
+    from paper_2508_13986_b200 import binding
+    cfg = W.config2()
+    cfg.update(thresh=1e-5, max_cells=1 << 20)
+    need = binding.arena_bytes(cfg["n"], cfg["max_cells"])
+    arena = torch.empty(need, dtype=torch.uint8, device="cuda")
+    free0 = torch.cuda.mem_get_info()[0]
+    ga = G(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfg["cfl"], max_cells=cfg["max_cells"], arena=arena)
+    assert free0 - torch.cuda.mem_get_info()[0] < (8 << 20)         # nothing of that size was allocated behind our back
+    gm = G(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], cfl=cfg["cfl"], max_cells=cfg["max_cells"])
+    for g in (ga, gm):
+        g.init_gaussian(cfg["mean"], cfg["cov"])
+        assert g.run(1e300, max_steps=7, prune_every=3) == 7
+    ka, pa = ga.export(); km, pm = gm.export()
+    assert np.array_equal(ka, km) and np.max(np.abs(pa - pm)) <= 1e-12 * pm.max()
+    ga.close(); gm.close()
+    with pytest.raises(binding.GbeesError) as ei:
+        G(cfg["n"], cfg["dx"], cfg["thresh"], cfg["dyn"], cfg["params"], max_cells=cfg["max_cells"], arena=arena[: need // 2])
+    assert ei.value.code == -4
+
+
 def test_marginals_of_the_6d_pdf():
     """f3: the two 3-D marginals of the 6-D Lorenz '96 PDF (and a 1-D, a 2-D one with
     permuted dimensions) by device hash-accumulation against the numpy group-by of the exported state."""
