@@ -257,7 +257,6 @@ __device__ void phase_targets(const Params& p, const Store& st, DevState* ds) {
                     sDiag[w][t - ND] = sl ? p11 >> w2 : p11 << w2;
                 }
             }
-            if (!__any_sync(0xffffffffu, (vOwn | v1 | v2) != 0ull)) continue;
 #pragma unroll
             for (int d = 0; d <= ND; ++d) {
                 const unsigned long long x = d == OWN ? vOwn : ((d == d1 ? v1 : 0ull) | (d == d2 ? v2 : 0ull));
