@@ -212,7 +212,7 @@ def run_cfg4(args):
                       "expected_probes": "PAPER.md:192: hit (1+1/(1-a))/2, miss (1+1/(1-a)^2)/2", "rows": rows}))
 
 
-KERNEL_OF_PHASE = {"grow": "k_detect + k_grow<{n},{d}>", "link": "k_link<{n},false>", "passA": "k_flux1<{n},{d},true>",
+KERNEL_OF_PHASE = {"grow": "k_detect + k_grow<{n},{d},skip>", "link": "k_link<{n},false>", "passA": "k_flux1<{n},{d},true>",
                    "passB": "k_flux2<{n}>", "mark": "k_mark<{n},{d}>", "compact": "k_prune_scan + k_prune_move + k_zero_tail",
                    "rebuild": "k_clear_table + k_prune_tail<{n},{d}>", "relink": "k_link_finish<{n}>", "correct": "k_correct<{n}>",
                    "run": "k_run_small<{n},{d},true>"}

@@ -45,8 +45,8 @@ __global__ void k_begin_run(DevState* ds, double t_target, unsigned long long st
 }
 __global__ void k_set_prune_ok(DevState* ds) { ds->prune_ok = 1; }
 __global__ void __launch_bounds__(TPB) k_detect(GP) { GUARD(1); ST; phase_detect(p, st, ds); }
-template <int NDIM, int DYN>
-__global__ void __launch_bounds__(TPB) k_grow(GP) { GUARD(1); ST; phase_targets<NDIM, DYN, true>(p, st, ds); }
+template <int NDIM, int DYN, bool SKIP>
+__global__ void __launch_bounds__(TPB) k_grow(GP) { GUARD(1); ST; phase_targets<NDIM, DYN, true, SKIP>(p, st, ds); }
 template <int NDIM, int DYN>
 __global__ void __launch_bounds__(TPB) k_mark(GP) { GUARD(2); ST; phase_targets<NDIM, DYN, false>(p, st, ds); }
 template <int NDIM, bool ALL>
@@ -159,7 +159,7 @@ __global__ void __launch_bounds__(TPB) k_run_small(GP, int prune_every, int no_g
         if (!no_grow) {
             phase_detect(p, st, ds);
             cl.sync();
-            phase_targets<NDIM, DYN, true>(p, st, ds);
+            phase_targets<NDIM, DYN, true, false>(p, st, ds);
             cl.sync();
             phase_link<NDIM, false>(p, st, ds);
             cl.sync();
@@ -716,7 +716,9 @@ static int enqueue_step(gbees_ctx* c) {
         if (!c->no_grow) {
             phase(c, GBEES_PH_GROW, 2, [&] {
                 kl(c, k_detect, c->grid, TPB, 0, c->p, c->st, c->d_st);
-                kl(c, k_grow<NN, DD>, c->grid, TPB, 0, c->p, c->st, c->d_st);
+                // (large grids list more source bricks than warps fit: throughput variant; small ones: latency variant)
+                if (c->h_st->NB > 65536u) kl(c, k_grow<NN, DD, true>, c->grid, TPB, 0, c->p, c->st, c->d_st);
+                else kl(c, k_grow<NN, DD, false>, c->grid, TPB, 0, c->p, c->st, c->d_st);
             });
             phase(c, GBEES_PH_LINK, 1, [&] { kl(c, k_link<NN, false>, c->grid, TPB, 0, c->p, c->st, c->d_st, 1); });
         }

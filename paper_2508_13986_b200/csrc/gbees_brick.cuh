@@ -146,7 +146,10 @@ __device__ inline void phase_detect(const Params& p, const Store& st, DevState* 
     }
 }
 
-template <int NDIM, int DYN, bool GROW>
+// SKIP: a class iteration in which no lane has a part is skipped. That pays when the pass is throughput-bound (mark;
+// grow on large grids); without the branch the three iterations overlap, which pays when one warp's latency is the
+// bound (grow on small grids: a few thousand listed bricks, one warp each).
+template <int NDIM, int DYN, bool GROW, bool SKIP = true>
 __device__ void phase_targets(const Params& p, const Store& st, DevState* ds) {
     using G = Geo<NDIM>;
     constexpr int ND = 2 * NDIM, NT = ND + 2 * NDIM * (NDIM - 1), OWN = ND;
@@ -257,6 +260,7 @@ __device__ void phase_targets(const Params& p, const Store& st, DevState* ds) {
                     sDiag[w][t - ND] = sl ? p11 >> w2 : p11 << w2;
                 }
             }
+            if (SKIP && !__any_sync(0xffffffffu, (vOwn | v1 | v2) != 0ull)) continue;
 #pragma unroll
             for (int d = 0; d <= ND; ++d) {
                 const unsigned long long x = d == OWN ? vOwn : ((d == d1 ? v1 : 0ull) | (d == d2 ? v2 : 0ull));
