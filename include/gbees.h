@@ -14,6 +14,9 @@
  *  - "host" / "device" below says where a pointer must live. Arrays passed in are copied; the
  *    caller keeps ownership of everything it passes. One context = one stream; calls on one
  *    context are not re-entrant.
+ *  - The kernels of a step / prune are enqueued with programmatic dependent launch (the next kernel's blocks are
+ *    scheduled while the previous one drains; every kernel waits for its predecessor before it reads anything).
+ *    Environment variable GBEES_NO_PDL=1 (read by gbees_create) switches that off, for measurement.
  *  - Cell c in Z^n has centre x_c = origin + c o dx; origin = the mean given to init_gaussian.
  *    P_c is the probability MASS of cell c; sum over active cells = 1 after every normalisation.
  */
