@@ -711,8 +711,13 @@ __device__ void phase_flux1(const Params& p, const Store& st, DevState* ds) {
             for (int j = 0; j < NDIM; ++j) {
                 const int s = 1 << G::SH(j), MK = G::MK(j);
                 const int lj = (l >> G::SH(j)) & MK;
-                if (lj < MK) v -= sm.Fb[j][FG::fb(j, l)];
-                if (lj > 0) v += sm.Fb[j][FG::fb(j, l - s)];
+                if (G::K(j) == 1) {     // two cells along j: the one in-brick face, entered under its lower cell's slot
+                    const double f = sm.Fb[j][FG::fb(j, l & ~s)];
+                    v += lj ? f : -f;
+                } else {
+                    if (lj < MK) v -= sm.Fb[j][FG::fb(j, l)];
+                    if (lj > 0) v += sm.Fb[j][FG::fb(j, l - s)];
+                }
             }
             st.Qn[(size_t)b * 64 + l] = on ? v : 0.0;
             st.fetch[(size_t)b * 64 + l] = on ? sm.fl[l] : (uint16_t)0;
