@@ -541,7 +541,6 @@ __device__ void phase_flux1(const Params& p, const Store& st, DevState* ds) {
                 }
             }
     }
-    // coordinate-table entry t of this lane: dimension tj, local index ti (entries beyond the table: tj = -1)
     constexpr uint32_t zrow = NBR_NONE;                     // missing neighbour brick: its staged row is zero-filled
     const uint64_t qlane = reinterpret_cast<uint64_t>(Q) + 16ull * lane;
     // metadata of the warp's next brick, loaded one brick ahead
