@@ -167,6 +167,26 @@ int gbees_marginal(gbees_ctx* ctx, const int* dims, int m, int32_t* keys, double
  * compare it with a run on that grid (gbees_compare). The context is not modified. */
 int gbees_resample(gbees_ctx* ctx, const double* origin2, const double* dx2, int32_t* keys, double* p, int64_t cap, int64_t* count);
 
+/* Marginal PDF WITHOUT ANY ALLOCATION (for callers that cannot call cudaMalloc: code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid it). Same result as gbees_marginal, but computed from an
+ * exported state instead of a context: keys [count_in*n] int32 row-major and p [count_in] (DEVICE pointers on
+ * `device`, e.g. what gbees_export wrote into device buffers), dims [m] (host; distinct indices in [0, n), output
+ * order = order in dims). Writes *count (host) marginal cells in unspecified order to out_keys [cap*m] int32 and
+ * out_p [cap] (DEVICE pointers, caller-owned). The scratch hashtable lives in a file-scope device array of
+ * 2 * GBEES_NOALLOC_MAX_CELLS slots (4 MiB, held by every GPU that loads the library until the process exits):
+ * count_in > GBEES_NOALLOC_MAX_CELLS is rejected with GBEES_ERR_CAPACITY (use gbees_marginal), cap < *count gives
+ * GBEES_ERR_BUFFER (with *count set), a kept coordinate outside floor(63/m) bits GBEES_ERR_KEY_RANGE. The call
+ * enqueues three kernels on `stream` (a cudaStream_t, NULL = default) and waits for them; it calls no cudaMalloc,
+ * cudaFree or allocating library routine. ALL calls share the one scratch array, which keeps the previous call's
+ * contents (each call clears what it uses first): calls that overlap on the GPU -- two streams, two threads -- RACE;
+ * serialise them. The additions are atomic, so the last bits of p may differ between calls.
+ * gbees_marginal_noalloc_error(): message of the calling thread's last failed call. */
+#define GBEES_NOALLOC_MAX_CELLS 131072
+int gbees_marginal_noalloc(int device, void* stream, int n, const int32_t* keys /*device*/, const double* p /*device*/,
+                           int64_t count_in, const int* dims /*host*/, int m, int32_t* out_keys /*device*/,
+                           double* out_p /*device*/, int64_t cap, int64_t* count /*host*/);
+const char* gbees_marginal_noalloc_error(void);
+
 /* Write the active cells in unspecified order: keys [cap*n] int32 row-major, p [cap] (normalised).
  * Buffers: host or device (detected), caller-owned. keys == NULL and p == NULL: only *count.
  * cap < count: nothing written, *count = needed, GBEES_ERR_BUFFER. count: host pointer. */

@@ -44,6 +44,23 @@ def arena_bytes(n, max_cells=1 << 20, load_factor=0.5):
     return b.value
 
 
+NOALLOC_MAX_CELLS = 131072   # GBEES_NOALLOC_MAX_CELLS in include/gbees.h
+
+
+def marginal_noalloc(keys_t, p_t, dims, out_keys_t, out_p_t, device=0, stream=None):
+    """gbees_marginal_noalloc: marginal of an exported state held in torch CUDA tensors (keys int32 [N, n],
+    p float64 [N]) into caller-owned CUDA tensors (int32 [cap, m], float64 [cap]); nothing is allocated.
+    Returns the number of marginal cells written."""
+    d = (C.c_int * len(dims))(*[int(x) for x in dims])
+    cnt = C.c_int64()
+    rc = lib().gbees_marginal_noalloc(int(device), C.c_void_p(stream) if stream else None, int(keys_t.shape[1]),
+                                      keys_t.data_ptr(), p_t.data_ptr(), int(p_t.numel()), d, len(dims),
+                                      out_keys_t.data_ptr(), out_p_t.data_ptr(), int(out_p_t.numel()), C.byref(cnt))
+    if rc:
+        raise GbeesError(rc, lib().gbees_marginal_noalloc_error().decode())
+    return cnt.value
+
+
 def lib_path():
     return _LIB_PATH
 
@@ -77,6 +94,9 @@ def lib():
         L.gbees_resample.argtypes = [vp, dp, dp, vp, vp, C.c_int64, C.POINTER(C.c_int64)]
         L.gbees_stats.argtypes = [vp, C.POINTER(Stats)]
         L.gbees_profile.argtypes = [vp, C.c_int, dp, C.POINTER(C.c_int64)]
+        L.gbees_marginal_noalloc.argtypes = [C.c_int, vp, C.c_int, vp, vp, C.c_int64, C.POINTER(C.c_int), C.c_int, vp, vp,
+                                             C.c_int64, C.POINTER(C.c_int64)]
+        L.gbees_marginal_noalloc_error.restype = C.c_char_p
         L.gbees_last_error.argtypes = [vp]
         L.gbees_last_error.restype = C.c_char_p
         L.gbees_clear_error.argtypes = [vp]

@@ -5,7 +5,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgbees.so")
-SOURCES = [os.path.join(CSRC, "gbees_api.cu"), os.path.join(CSRC, "gbees_ht.cu")]
+SOURCES = [os.path.join(CSRC, "gbees_api.cu"), os.path.join(CSRC, "gbees_ht.cu"), os.path.join(CSRC, "gbees_noalloc.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("gbees_common.cuh", "gbees_prims.cuh", "gbees_brick.cuh")] + [
     os.path.join(os.path.dirname(HERE), "include", "gbees.h")]
 
