@@ -588,7 +588,7 @@ int gbees_create(gbees_ctx** out, int n, const double* dx, double threshold, int
     // dynamic shared memory above 48 KB is an opt-in per function AND per device: set it for this context's device
     if (dispatch(c, [&](auto N_, auto D_) {
             constexpr int NN = decltype(N_)::value, DD = decltype(D_)::value;
-            constexpr int smem = (int)(sizeof(Flux1Smem<NN>) * FLUX1_WPB);
+            constexpr int smem = (int)(sizeof(Flux1Warp<NN>) * FLUX1_WPB);
             if (cudaFuncSetAttribute(k_flux1<NN, DD, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess ||
                 cudaFuncSetAttribute(k_flux1<NN, DD, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
                 return GBEES_ERR_CUDA;
@@ -723,7 +723,7 @@ static int enqueue_step(gbees_ctx* c) {
             phase(c, GBEES_PH_LINK, 1, [&] { kl(c, k_link<NN, false>, c->grid, TPB, 0, c->p, c->st, c->d_st, 1); });
         }
         phase(c, GBEES_PH_PASSA, 1, [&] {
-            constexpr size_t smem = sizeof(Flux1Smem<NN>) * FLUX1_WPB;   // opt-in above 48 KB: set per device in gbees_create
+            constexpr size_t smem = sizeof(Flux1Warp<NN>) * FLUX1_WPB;   // opt-in above 48 KB: set per device in gbees_create
             if (c->p.hi_res && !c->p.limiter) kl(c, k_flux1<NN, DD, true>, c->grid_flux1, 32 * FLUX1_WPB, smem, c->p, c->st, c->d_st);
             else kl(c, k_flux1<NN, DD, false>, c->grid_flux1, 32 * FLUX1_WPB, smem, c->p, c->st, c->d_st);
         });
@@ -1049,7 +1049,7 @@ constexpr uint32_t SMALL_NB_ENTER = 256, SMALL_NB_LEAVE = 512;
 static int launch_small(gbees_ctx* c, int prune_every, unsigned long long k_start) {
     int rc = dispatch(c, [&](auto N_, auto D_) {
         constexpr int NN = decltype(N_)::value, DD = decltype(D_)::value;
-        constexpr size_t smem = sizeof(Flux1Smem<NN>) * WPB;
+        constexpr size_t smem = sizeof(Flux1Warp<NN>) * WPB;
         const bool fast = c->p.hi_res && !c->p.limiter;
         auto kern = fast ? k_run_small<NN, DD, true, false> : k_run_small<NN, DD, false, false>;
         if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return GBEES_ERR_CUDA;
@@ -1073,7 +1073,7 @@ static int launch_small(gbees_ctx* c, int prune_every, unsigned long long k_star
 static int launch_coop(gbees_ctx* c, int prune_every, unsigned long long k_start) {
     return dispatch(c, [&](auto N_, auto D_) {
         constexpr int NN = decltype(N_)::value, DD = decltype(D_)::value;
-        constexpr size_t smem = sizeof(Flux1Smem<NN>) * WPB;
+        constexpr size_t smem = sizeof(Flux1Warp<NN>) * WPB;
         const bool fast = c->p.hi_res && !c->p.limiter;
         auto kern = fast ? k_run_small<NN, DD, true, true> : k_run_small<NN, DD, false, true>;
         if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return GBEES_ERR_CUDA;

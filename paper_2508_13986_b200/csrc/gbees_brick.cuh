@@ -451,23 +451,40 @@ struct FluxGeo {
     // face array: one entry per in-brick face and dimension, addressed by the slot of the face's LOWER cell
     // (64 entries per dimension; packing them to the 32 that a two-cell-wide dimension uses costs more index
     // arithmetic per cell than the shared memory is worth while registers cap the occupancy at 2 blocks per SM)
-    static constexpr int FB = 64;
-    __host__ __device__ static constexpr int fb(int, int l) { return l; }
+    // every dimension two cells wide (n = 6): only HALF of each neighbour row is ever read -- the cells that face
+    // this brick -- so the two neighbour rows of a dimension are staged as ONE combined row (see Flux1Smem::R)
+    __host__ __device__ static constexpr bool all_two() { for (int j = 0; j < NDIM; ++j) if (G::K(j) != 1) return false; return true; }
+    static constexpr bool ALL2 = all_two();
+    // (ALL2: a dimension has 32 in-brick faces, entered under the slot of the lower cell with bit j removed)
+    static constexpr int FB = ALL2 ? 32 : 64;
+    __host__ __device__ static constexpr int fb(int j, int l) { return ALL2 ? G::fidx(j, l) : l; }
 };
 
 // Shared memory of one warp in pass 1
 template <int NDIM>
 struct alignas(16) Flux1Smem {
-    static constexpr int ROWS = 2 * NDIM + 1, OWN = 2 * NDIM;
-    double R[ROWS][64];              // staged rows: 2n neighbour bricks, then the brick itself
+    // staged rows. General geometry: the 2n neighbour bricks' rows (index d = 2j + side), then the brick's own row.
+    // ALL2 geometry: one combined row per dimension j -- slot l' holds the value of the cell at slot l' of the
+    // LOWER neighbour brick if bit j of l' is set (it is the lower neighbour of the own cell l' ^ s), of the UPPER
+    // neighbour brick if the bit is clear (the upper neighbour of l' ^ s) -- then the own row: n + 1 rows, not 2n + 1.
+    static constexpr bool ALL2 = FluxGeo<NDIM>::ALL2;
+    static constexpr int ROWS = ALL2 ? NDIM + 1 : 2 * NDIM + 1, OWN = ROWS - 1;
+    double R[ROWS][64];
     double Fb[NDIM][FluxGeo<NDIM>::FB];   // F through the UPPER j-face of slot l, faces inside the brick only
     double acc[64];                  // P_c minus / plus the fluxes the cell applied to itself
     double xc[FluxGeo<NDIM>::NC];    // cell-centre coordinates per dimension and local index
     double xf[FluxGeo<NDIM>::NF];    // face coordinates: entry i = lower face of local index i
     unsigned long long A[2 * NDIM];  // bit l of A[d]: the neighbour of slot l in direction d is active
     unsigned long long RZ[2 * NDIM]; // bit l of RZ[d]: slot l active, that neighbour NOT active, the cell behind it active
+    uint32_t adjr[2 * NDIM];         // rows of the 2n neighbour bricks (ALL2: two-hop values are read from global memory)
     uint16_t fl[64];
-    uint8_t list[64];
+};
+// Shared memory of one warp in pass 1: NBW bricks in flight and their common cell list ((brick << 6) | slot)
+template <int NDIM>
+struct alignas(16) Flux1Warp {
+    static constexpr int NBW = FluxGeo<NDIM>::ALL2 ? 2 : 1;
+    Flux1Smem<NDIM> b[NBW];
+    uint8_t list[64 * NBW];
 };
 
 // A_j and B_j of f_j = A_j + B_j x_j (operation order fixed by the explicit intrinsics)
@@ -512,10 +529,14 @@ __device__ void phase_flux1(const Params& p, const Store& st, DevState* ds) {
     using G = Geo<NDIM>;
     using FG = FluxGeo<NDIM>;
     using SM = Flux1Smem<NDIM>;
-    constexpr int ND = 2 * NDIM, OWN = SM::OWN;
+    constexpr int ND = 2 * NDIM, OWN = SM::OWN, LOWN = ND;   // OWN: staged row of the brick itself; LOWN: the lane that holds its row / mask
+    constexpr bool ALL2 = SM::ALL2;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const unsigned w = threadIdx.x >> 5, lane = lane_id();
-    SM& sm = reinterpret_cast<SM*>(smem_raw)[w];
+    constexpr int NBW = Flux1Warp<NDIM>::NBW;
+    Flux1Warp<NDIM>& ws = reinterpret_cast<Flux1Warp<NDIM>*>(smem_raw)[w];
+    SM* const smw = ws.b;
+    uint8_t* const wlist = ws.list;
     const uint32_t NB = min(ds->NB, p.capB);
     const double dt = step_dt(p, ds);
     const bool hires = FAST || p.hi_res != 0, nolim = !FAST && p.limiter != 0;
@@ -543,37 +564,73 @@ __device__ void phase_flux1(const Params& p, const Store& st, DevState* ds) {
     }
     constexpr uint32_t zrow = NBR_NONE;                     // missing neighbour brick: its staged row is zero-filled
     const uint64_t qlane = reinterpret_cast<uint64_t>(Q) + 16ull * lane;
-    // metadata of the warp's next brick, loaded one brick ahead
-    uint32_t nx_row = zrow;
-    uint64_t nx_mask = 0ull, nx_bk = 0ull;
-    auto fetch_rows = [&](uint32_t bb) {   // (nothing here may USE what it loads: the loads stay in flight behind the cell loop)
-        nx_row = zrow;
-        if (bb < NB) {
-            if (lane < ND) nx_row = st.adj[(size_t)bb * ND + lane];     // NBR_NONE = zrow: a missing neighbour
-            else if (lane == OWN) nx_row = bb;
-            nx_bk = st.bkey[bb];
+    // A warp works on NBW bricks at a time: their active cells go into ONE list that is worked off 32 cells at a
+    // time, whichever brick a cell belongs to (a brick holds 20-38 active cells: one brick at a time leaves 25-45 %
+    // of the lanes of its last iteration idle). Two bricks fit in shared memory only with the combined rows.
+    // Metadata of the warp's next NBW bricks is loaded one round ahead.
+    uint32_t nx_row[NBW];
+    uint64_t nx_mask[NBW], nx_bk[NBW];
+    auto fetch_rows = [&](uint32_t b0) {   // (nothing here may USE what it loads: the loads stay in flight behind the cell loop)
+#pragma unroll
+        for (int u = 0; u < NBW; ++u) {
+            const uint32_t bb = b0 + u * gwarps();
+            nx_row[u] = zrow; nx_bk[u] = 0ull;
+            if (bb < NB) {
+                if (lane < ND) nx_row[u] = st.adj[(size_t)bb * ND + lane];     // NBR_NONE = zrow: a missing neighbour
+                else if (lane == LOWN) nx_row[u] = bb;
+                nx_bk[u] = st.bkey[bb];
+            }
         }
     };
-    auto fetch_masks = [&]() { nx_mask = (lane <= OWN && nx_row != zrow) ? st.mask[nx_row] : 0ull; };
+    auto fetch_masks = [&]() {
+#pragma unroll
+        for (int u = 0; u < NBW; ++u) nx_mask[u] = (lane <= LOWN && nx_row[u] != zrow) ? st.mask[nx_row[u]] : 0ull;
+    };
     fetch_rows(gwarp());
     fetch_masks();
     unsigned ncells = 0;                                    // active cells of this warp's bricks (the grow does not count)
-    for (uint32_t b = gwarp(); b < NB; b += gwarps()) {   // warp-uniform
+    for (uint32_t b0 = gwarp(); b0 < NB; b0 += NBW * gwarps()) {   // warp-uniform
+        uint64_t mu[NBW];                                   // active masks of the round's bricks (0: no such brick)
+        int cbase[NBW + 1];                                 // their ranges in the cell list
+        cbase[0] = 0;
+#pragma unroll
+        for (int u = 0; u < NBW; ++u) {
+        SM& sm = smw[u];
+        const uint32_t b = b0 + u * gwarps();
+        if (b >= NB) { mu[u] = 0ull; cbase[u + 1] = cbase[u]; continue; }
         // ---- stage the 2n+1 rows (LDGSTS: 16 bytes per lane = one 512-byte row per warp instruction,
         // no register round trip); a missing neighbour brick is zero-filled by the same instruction.
-        const uint32_t my_row = nx_row;
-        const uint64_t my_mask = nx_mask, bk = nx_bk;
+        const uint32_t my_row = nx_row[u];
+        const uint64_t my_mask = nx_mask[u], bk = nx_bk[u];
+        // (a missing brick copies nothing and zero-fills: the source address is then only a placeholder)
+        if (ALL2) {
+            // one combined row per dimension: lane L copies the 16-byte chunk of slots 2L, 2L + 1 from the lower
+            // neighbour's row if bit j of those slots is set, from the upper neighbour's row otherwise; in the last
+            // dimension (stride 1) the two slots of a chunk differ in that bit: two 8-byte copies
 #pragma unroll
-        for (int r = 0; r < SM::ROWS; ++r) {
-            const uint32_t row = __shfl_sync(0xffffffffu, my_row, r);
-            // (a missing brick copies nothing and zero-fills: the source address is only a placeholder)
-            __pipeline_memcpy_async(&sm.R[r][2 * lane], reinterpret_cast<const void*>(qlane + (uint64_t)(row == NBR_NONE ? b : row) * 512ull), 16, row == NBR_NONE ? 16 : 0);
+            for (int j = 0; j < NDIM; ++j) {
+                if (G::SH(j) >= 1) {
+                    const int side = (((2 * (int)lane) >> G::SH(j)) & 1) ? 0 : 1;       // 0: lower neighbour (d = 2j), 1: upper
+                    const uint32_t row = __shfl_sync(0xffffffffu, my_row, 2 * j + side);
+                    __pipeline_memcpy_async(&sm.R[j][2 * lane], reinterpret_cast<const void*>(qlane + (uint64_t)(row == NBR_NONE ? b : row) * 512ull), 16, row == NBR_NONE ? 16 : 0);
+                } else {
+                    const uint32_t rl = __shfl_sync(0xffffffffu, my_row, 2 * j), ru = __shfl_sync(0xffffffffu, my_row, 2 * j + 1);
+                    __pipeline_memcpy_async(&sm.R[j][2 * lane], reinterpret_cast<const void*>(qlane + (uint64_t)(ru == NBR_NONE ? b : ru) * 512ull), 8, ru == NBR_NONE ? 8 : 0);
+                    __pipeline_memcpy_async(&sm.R[j][2 * lane + 1], reinterpret_cast<const void*>(qlane + 8ull + (uint64_t)(rl == NBR_NONE ? b : rl) * 512ull), 8, rl == NBR_NONE ? 8 : 0);
+                }
+            }
+            __pipeline_memcpy_async(&sm.R[OWN][2 * lane], reinterpret_cast<const void*>(qlane + (uint64_t)b * 512ull), 16);
+            if (lane < ND) sm.adjr[lane] = my_row;
+        } else {
+#pragma unroll
+            for (int r = 0; r < SM::ROWS; ++r) {
+                const uint32_t row = __shfl_sync(0xffffffffu, my_row, r);
+                __pipeline_memcpy_async(&sm.R[r][2 * lane], reinterpret_cast<const void*>(qlane + (uint64_t)(row == NBR_NONE ? b : row) * 512ull), 16, row == NBR_NONE ? 16 : 0);
+            }
         }
-        __pipeline_commit();
-        fetch_rows(b + gwarps());                           // next brick: rows now, masks after the cell loop
         // ---- while the rows are in flight: activity masks, coordinate tables, face array, cell list
-        const uint64_t m = ((uint64_t)__shfl_sync(0xffffffffu, (uint32_t)(my_mask >> 32), OWN) << 32) |
-                           __shfl_sync(0xffffffffu, (uint32_t)my_mask, OWN);
+        const uint64_t m = ((uint64_t)__shfl_sync(0xffffffffu, (uint32_t)(my_mask >> 32), LOWN) << 32) |
+                           __shfl_sync(0xffffffffu, (uint32_t)my_mask, LOWN);
         if (lane < ND) {
             const bool up = lane & 1;
             const unsigned long long a1 = ((up ? m >> my_s : m << my_s) & ~my_edge) |
@@ -602,34 +659,46 @@ __device__ void phase_flux1(const Params& p, const Store& st, DevState* ds) {
             if (2 * (int)lane < FG::FB) *reinterpret_cast<double2*>(&sm.Fb[j][2 * lane]) = make_double2(0.0, 0.0);
         const uint32_t m_lo = (uint32_t)m, m_hi = (uint32_t)(m >> 32);
         const uint32_t below = (1u << lane) - 1u;
-        if ((m_lo >> lane) & 1u) sm.list[__popc(m_lo & below)] = (uint8_t)lane;
-        if ((m_hi >> lane) & 1u) sm.list[__popc(m_lo) + __popc(m_hi & below)] = (uint8_t)(lane + 32);
-        const int cnt = __popcll(m);
+        if ((m_lo >> lane) & 1u) wlist[cbase[u] + __popc(m_lo & below)] = (uint8_t)((u << 6) | lane);
+        if ((m_hi >> lane) & 1u) wlist[cbase[u] + __popc(m_lo) + __popc(m_hi & below)] = (uint8_t)((u << 6) | (lane + 32));
+        mu[u] = m;
+        cbase[u + 1] = cbase[u] + __popcll(m);
+        }
+        __pipeline_commit();
+        fetch_rows(b0 + NBW * gwarps());                    // next round: rows now, masks after the cell loop
+        const int cnt = cbase[NBW];
         ncells += (unsigned)cnt;
         __pipeline_wait_prior(0);
         __syncwarp();
-        const double* Rf = &sm.R[0][0];
         // ---- cell loop: active cells, 32 at a time
         for (int r0 = 0; r0 < cnt; r0 += 32) {
             if (r0 + (int)lane >= cnt) continue;
-            const int l = sm.list[r0 + lane];
-            const double q0 = sm.R[OWN][l];
+            const unsigned e = wlist[r0 + lane];
+            const int l = (int)(e & 63u);
+            SM& cs = smw[NBW > 1 ? (e >> 6) : 0];           // the cell's brick
+            const uint32_t b = b0 + (NBW > 1 ? (e >> 6) : 0u) * gwarps();
+            const double* Rf = &cs.R[0][0];
+            const double q0 = cs.R[OWN][l];
             const unsigned lbit = 1u << (l & 31);
-            const unsigned* Aw = reinterpret_cast<const unsigned*>(&sm.A[0]) + (l >> 5);    // this cell's half of every mask
-            const unsigned* Zw = reinterpret_cast<const unsigned*>(&sm.RZ[0]) + (l >> 5);
+            const unsigned* Aw = reinterpret_cast<const unsigned*>(&cs.A[0]) + (l >> 5);    // this cell's half of every mask
+            const unsigned* Zw = reinterpret_cast<const unsigned*>(&cs.RZ[0]) + (l >> 5);
             double x[NDIM], al[NDIM], au[NDIM], dm[NDIM], dp[NDIM], T[NDIM];
 #pragma unroll
-            for (int j = 0; j < NDIM; ++j) x[j] = sm.xc[FG::XC(j) + ((l >> G::SH(j)) & G::MK(j))];
+            for (int j = 0; j < NDIM; ++j) x[j] = cs.xc[FG::XC(j) + ((l >> G::SH(j)) & G::MK(j))];
             double S = 0.0;
 #pragma unroll
             for (int j = 0; j < NDIM; ++j) {
                 const int s = 1 << G::SH(j), MK = G::MK(j);
                 const int lj = (l >> G::SH(j)) & MK;
                 const double tA = __dmul_rn(tau[j], (dyn_A<NDIM, DYN>(p, x, j)));
-                al[j] = __fma_rn(tauB[j], sm.xf[FG::XF(j) + lj], tA);
-                au[j] = __fma_rn(tauB[j], sm.xf[FG::XF(j) + lj + 1], tA);
+                al[j] = __fma_rn(tauB[j], cs.xf[FG::XF(j) + lj], tA);
+                au[j] = __fma_rn(tauB[j], cs.xf[FG::XF(j) + lj + 1], tA);
                 double vm, vp;
-                if (G::K(j) == 1) {                // two cells along j: both neighbours sit at slot l ^ s, in the own row or across the face
+                if (ALL2) {                        // both neighbours sit at slot l ^ s: one in the own row, one in the combined row j
+                    const double v_in = Rf[OWN * 64 + (l ^ s)], v_out = Rf[j * 64 + (l ^ s)];
+                    vm = lj ? v_in : v_out;
+                    vp = lj ? v_out : v_in;
+                } else if (G::K(j) == 1) {         // two cells along j: both neighbours sit at slot l ^ s, in the own row or across the face
                     const double* nb = Rf + (l ^ s);
                     vm = nb[(lj ? OWN : 2 * j) * 64];
                     vp = nb[(lj ? 2 * j + 1 : OWN) * 64];
@@ -659,7 +728,7 @@ __device__ void phase_flux1(const Params& p, const Store& st, DevState* ds) {
                     if (dpos(a)) {
                         const double wv = hires ? (nolim ? dp[j] : sig) : 0.0;
                         const double F = a * fma(0.5 - 0.5 * a, wv, Gj);
-                        if (lj < MK) sm.Fb[j][FG::fb(j, l)] = F;
+                        if (lj < MK) cs.Fb[j][FG::fb(j, l)] = F;
                         else {
                             part -= F;
                             if (Aw[2 * (2 * j + 1)] & lbit) st.phi[((size_t)b * ND + 2 * j + 1) * 32 + G::fidx(j, l)] = F;
@@ -668,8 +737,11 @@ __device__ void phase_flux1(const Params& p, const Store& st, DevState* ds) {
                         if (lj == MK && (Aw[2 * (2 * j + 1)] & lbit)) fl |= 1u << (2 * j + 1);
                         // upwind cell c+e^j inactive: W = 0 - P_c, W_up = P_{c+2e^j} - 0 (zero unless c+2e^j is active)
                         if (hires && (Zw[2 * (2 * j + 1)] & lbit)) {
-                            const int i2 = lj + 2 <= MK ? OWN * 64 + l + 2 * s : (2 * j + 1) * 64 + l + (1 - MK) * s;
-                            const double wv = nolim ? dp[j] : mc_limit_fast(dp[j], Rf[i2]);
+                            double v2;                   // P_{c+2e^j}
+                            if (nolim) v2 = 0.0;          // (not used without a limiter, and the cell behind need not exist then)
+                            else if (ALL2) v2 = lj ? Q[(size_t)cs.adjr[2 * j + 1] * 64 + l] : Rf[j * 64 + l];   // upper brick, slot l: staged only for lj = 0
+                            else v2 = Rf[lj + 2 <= MK ? OWN * 64 + l + 2 * s : (2 * j + 1) * 64 + l + (1 - MK) * s];
+                            const double wv = nolim ? dp[j] : mc_limit_fast(dp[j], v2);
                             part -= a * ((-0.5 - 0.5 * a) * wv);
                         }
                     }
@@ -679,7 +751,7 @@ __device__ void phase_flux1(const Params& p, const Store& st, DevState* ds) {
                     if (dneg(a)) {
                         const double wv = hires ? (nolim ? dm[j] : sig) : 0.0;
                         const double F = a * fma(-0.5 - 0.5 * a, wv, Gj);
-                        if (lj > 0) sm.Fb[j][FG::fb(j, l - s)] = F;
+                        if (lj > 0) cs.Fb[j][FG::fb(j, l - s)] = F;
                         else {
                             part += F;
                             if (Aw[2 * (2 * j)] & lbit) st.phi[((size_t)b * ND + 2 * j) * 32 + G::fidx(j, l)] = F;
@@ -688,19 +760,28 @@ __device__ void phase_flux1(const Params& p, const Store& st, DevState* ds) {
                         if (lj == 0 && (Aw[2 * (2 * j)] & lbit)) fl |= 1u << (2 * j);
                         // upwind cell c-e^j inactive: W = P_c - 0, W_up = 0 - P_{c-2e^j} (zero unless c-2e^j is active)
                         if (hires && (Zw[2 * (2 * j)] & lbit)) {
-                            const int i2 = lj - 2 >= 0 ? OWN * 64 + l - 2 * s : (2 * j) * 64 + l + (MK - 1) * s;
-                            const double wv = nolim ? dm[j] : mc_limit_fast(dm[j], -Rf[i2]);
+                            double v2;                   // P_{c-2e^j}
+                            if (nolim) v2 = 0.0;
+                            else if (ALL2) v2 = lj ? Rf[j * 64 + l] : Q[(size_t)cs.adjr[2 * j] * 64 + l];       // lower brick, slot l: staged only for lj = 1
+                            else v2 = Rf[lj - 2 >= 0 ? OWN * 64 + l - 2 * s : (2 * j) * 64 + l + (MK - 1) * s];
+                            const double wv = nolim ? dm[j] : mc_limit_fast(dm[j], -v2);
                             part += a * ((0.5 - 0.5 * a) * wv);
                         }
                     }
                 }
             }
-            sm.acc[l] = part;
-            sm.fl[l] = (uint16_t)fl;
+            cs.acc[l] = part;
+            cs.fl[l] = (uint16_t)fl;
         }
         fetch_masks();                                      // next brick (its rows were fetched above)
         __syncwarp();
         // ---- apply the in-brick face fluxes to both of their cells, write the partial update
+#pragma unroll
+        for (int u = 0; u < NBW; ++u) {
+        SM& sm = smw[u];
+        const uint32_t b = b0 + u * gwarps();
+        if (b >= NB) continue;
+        const uint64_t m = mu[u];
 #pragma unroll
         for (int hh = 0; hh < 2; ++hh) {
             const int l = (int)lane + 32 * hh;
@@ -720,6 +801,7 @@ __device__ void phase_flux1(const Params& p, const Store& st, DevState* ds) {
             }
             st.Qn[(size_t)b * 64 + l] = on ? v : 0.0;
             st.fetch[(size_t)b * 64 + l] = on ? sm.fl[l] : (uint16_t)0;
+        }
         }
         __syncwarp();
     }
